@@ -1,0 +1,180 @@
+"""ctypes binding of the CPU oracle (oracle/sp_oracle.c).
+
+TEST INFRASTRUCTURE.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this package; the product (paper_1104_3408_b200) never does.
+The oracle is plain C with long-double accumulation written from PAPER.md; see the header of
+sp_oracle.c for what each function follows and how it is pinned.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+_dp = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_ip = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        _lib.orc_wigner_d_sum.restype = C.c_double
+        _lib.orc_wigner_d_sum.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double]
+        _lib.orc_synthesis_matrix.restype = C.c_int
+        _lib.orc_ncomp.restype = C.c_int
+    return _lib
+
+
+def set_threads(n: int) -> None:
+    """Number of OpenMP threads the oracle may use (its loops over fields/spheres)."""
+    os.environ["OMP_NUM_THREADS"] = str(n)
+    try:
+        omp = C.CDLL("libgomp.so.1")
+        omp.omp_set_num_threads(int(n))
+    except OSError:
+        pass
+
+
+def grid(Nr, Nt, Np, rmin, rmax):
+    r, th, ph = np.zeros(Nr), np.zeros(Nt), np.zeros(Np)
+    lib().orc_grid(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_double(rmin), C.c_double(rmax),
+                   r.ctypes, th.ctypes, ph.ctypes)
+    return r, th, ph
+
+
+def cheb_diff(N, rmin, rmax):
+    D = np.zeros((N, N))
+    lib().orc_cheb_diff(C.c_int(N), C.c_double(rmin), C.c_double(rmax), D.ctypes)
+    return D
+
+
+def fourier_diff(n):
+    D = np.zeros((n, n))
+    lib().orc_fourier_diff(C.c_int(n), D.ctypes)
+    return D
+
+
+def _state(u, Nr, Nt, Np):
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    nf = u.size // (Nr * Nt * Np)
+    assert nf * Nr * Nt * Np == u.size
+    return u, nf
+
+
+def d_r(u, Nr, Nt, Np, rmin, rmax):
+    u, nf = _state(u, Nr, Nt, Np)
+    out = np.empty_like(u)
+    lib().orc_dr(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_int(nf), C.c_double(rmin), C.c_double(rmax),
+                 u.ctypes, out.ctypes)
+    return out
+
+
+def d_theta(u, Nr, Nt, Np):
+    u, nf = _state(u, Nr, Nt, Np)
+    out = np.empty_like(u)
+    lib().orc_dtheta(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_int(nf), u.ctypes, out.ctypes)
+    return out
+
+
+def d_phi(u, Nr, Nt, Np):
+    u, nf = _state(u, Nr, Nt, Np)
+    out = np.empty_like(u)
+    lib().orc_dphi(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_int(nf), u.ctypes, out.ctypes)
+    return out
+
+
+def gradient(u, Nr, Nt, Np, rmin, rmax):
+    """u: [nf, Np, Nt, Nr] (C order; r fastest) -> du: [3, nf, Np, Nt, Nr] = d/dx, d/dy, d/dz."""
+    u, nf = _state(u, Nr, Nt, Np)
+    du = np.empty((3, nf, Np, Nt, Nr))
+    lib().orc_gradient(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_int(nf), C.c_double(rmin), C.c_double(rmax),
+                       u.ctypes, du.ctypes)
+    return du
+
+
+def gradient_at(u, Nr, Nt, Np, rmin, rmax, samples):
+    """samples: int array [ns, 4] of (k, i, j, mu) -> [ns, 3] gradient values."""
+    u, nf = _state(u, Nr, Nt, Np)
+    s = np.ascontiguousarray(samples, dtype=np.int32)
+    out = np.empty((s.shape[0], 3))
+    lib().orc_gradient_at(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_int(nf), C.c_double(rmin), C.c_double(rmax),
+                          u.ctypes, C.c_int(s.shape[0]), s.ctypes, out.ctypes)
+    return out
+
+
+def wigner_d_sum(l, mp, m, th):
+    return lib().orc_wigner_d_sum(l, mp, m, float(th))
+
+
+def spin_P(n, m, lmax, th):
+    """P^n_{lm}(th) for l = 0..lmax (eq. 46)."""
+    out = np.zeros(lmax + 1)
+    lib().orc_spin_P(C.c_int(n), C.c_int(m), C.c_int(lmax), C.c_double(th), out.ctypes)
+    return out
+
+
+def synthesis_matrix(N, n, m):
+    l0 = max(abs(n), abs(m))
+    if N - l0 <= 0:
+        return np.zeros((N, 0))
+    P = np.zeros((N, N - l0))
+    lib().orc_synthesis_matrix(C.c_int(N), C.c_int(n), C.c_int(m), P.ctypes)
+    return P
+
+
+def filter_matrix(N, L, n, m):
+    F = np.zeros((N, N))
+    lib().orc_filter_matrix(C.c_int(N), C.c_int(L), C.c_int(n), C.c_int(m), F.ctypes)
+    return F
+
+
+def spin_analysis(N, n, m, s):
+    l0 = max(abs(n), abs(m))
+    s = np.ascontiguousarray(s, dtype=np.float64)
+    c = np.zeros(max(N - l0, 0))
+    lib().orc_spin_analysis(C.c_int(N), C.c_int(n), C.c_int(m), s.ctypes, c.ctypes)
+    return c
+
+
+def spin_filter_sphere(N, L, n, g):
+    """g: complex [J=2N, N] (index [j, i]) -> filtered complex array of the same shape."""
+    g = np.asarray(g)
+    gre = np.ascontiguousarray(g.real, dtype=np.float64)
+    gim = np.ascontiguousarray(g.imag if np.iscomplexobj(g) else np.zeros_like(gre), dtype=np.float64)
+    ore, oim = np.empty_like(gre), np.empty_like(gre)
+    lib().orc_spin_filter_sphere(C.c_int(N), C.c_int(L), C.c_int(n), gre.ctypes, gim.ctypes, ore.ctypes, oim.ctypes)
+    return ore + 1j * oim
+
+
+def ncomp(rank, dims, sym):
+    d = np.ascontiguousarray(list(dims) + [0] * (3 - len(dims)), dtype=np.int32)
+    return lib().orc_ncomp(C.c_int(rank), d.ctypes, C.c_int(sym[0]), C.c_int(sym[1]))
+
+
+def tensor_filter(u, Nr, Nt, Np, L, tensors, ksel=-1):
+    """Yn tensor filter.  tensors: list of dicts {rank, dims (len rank, 3|4), sym (a,b)|(-1,-1),
+    fields [stored components in canonical order]}.  Returns the filtered state (same shape);
+    fields in no tensor are copied through.  ksel >= 0: only that radius is filtered."""
+    u, nf = _state(u, Nr, Nt, Np)
+    out = np.empty_like(u)
+    nt = len(tensors)
+    rank = np.array([t["rank"] for t in tensors], dtype=np.int32)
+    dims = np.zeros((nt, 3), dtype=np.int32)
+    sym = np.full((nt, 2), -1, dtype=np.int32)
+    foff = np.zeros(nt + 1, dtype=np.int32)
+    fl = []
+    for q, t in enumerate(tensors):
+        for a, d in enumerate(t["dims"]):
+            dims[q, a] = d
+        sym[q] = t.get("sym", (-1, -1))
+        assert len(t["fields"]) == ncomp(t["rank"], t["dims"], sym[q]), "component count mismatch"
+        fl += list(t["fields"])
+        foff[q + 1] = len(fl)
+    fields = np.array(fl if fl else [0], dtype=np.int32)
+    lib().orc_tensor_filter(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_int(L), C.c_int(nf), u.ctypes, out.ctypes,
+                            C.c_int(nt), rank.ctypes, dims.ctypes, sym.ctypes, foff.ctypes, fields.ctypes,
+                            C.c_int(ksel))
+    return out
