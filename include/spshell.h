@@ -1,0 +1,123 @@
+/*
+ * spshell.h -- C ABI of the B200-native hot path of Bruegmann's CFF pseudospectral matrix method
+ * for tensor fields on a spherical shell (arXiv:1104.3408; citations are PAPER.md:<line>).
+ *
+ * The library computes, entirely in hand-written FP64 CUDA kernels for sm_100a,
+ *   (a) the Cartesian gradient of all evolved fields from the Chebyshev (radial) and double-Fourier
+ *       (theta, phi) differentiation matrices plus the coordinate Jacobian (eq. 6-19);
+ *   (b) the spin-weighted spherical-harmonic "Yn" tensor filter as matrix multiplication
+ *       (eq. 46-62);
+ *   (c) the right-hand side of the first-order scalar wave system with characteristic boundaries
+ *       (config 5 of BASELINE.json; readings W1-W3).
+ * There is no CPU fallback and no other backend: every hot call needs a CUDA device.
+ *
+ * STATE LAYOUT (PAPER.md:118 with the single cover, reading Q4).  Every state-shaped
+ * array is `double`, linear index
+ *        p = k + Nr*(i + Ntheta*(j + Nphi*mu)),
+ * k = radial node (fastest), i = latitude, j = longitude, mu = field (slowest).  Grid (eq. 2-4):
+ * r_k = (r_out+r_in)/2 - (r_out-r_in)/2 cos(pi k/(Nr-1)), theta_i = pi(i+1/2)/Ntheta,
+ * phi_j = 2 pi j/Nphi, with Nphi = 2 Ntheta (eq. 5).
+ *
+ * POINTERS.  Arguments named *_dev are DEVICE pointers owned by the caller (PyTorch allocations in
+ * the Python binding); *_host are host pointers.  The library owns only the sp_shell and the
+ * device-resident matrix tables it uploaded in sp_build_matrices.  Hot calls allocate nothing, are
+ * asynchronous on the given stream (a cudaStream_t passed as void*, NULL = default stream), do not
+ * synchronise, and are deterministic (no atomics): same inputs give bit-identical outputs.
+ *
+ * ERRORS.  Every call returns an sp_status; nothing throws across the ABI.
+ */
+#ifndef SPSHELL_H
+#define SPSHELL_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sp_shell sp_shell; /* opaque */
+
+typedef enum {
+    SP_OK = 0,
+    SP_ERR_INVALID_ARG = 1, /* Nphi != 2 Ntheta, Nr < 2, Ntheta < 2, r_out <= r_in, r_in <= 0, L < 0, L > Ntheta-1,
+                               null pointer, short workspace, rank > 3, malformed tensor descriptor */
+    SP_ERR_NOT_BUILT = 2,   /* a hot call before sp_build_matrices */
+    SP_ERR_ALLOC = 3,       /* host or device allocation failed */
+    SP_ERR_CUDA = 4,        /* a CUDA runtime call or kernel launch failed */
+    SP_ERR_UNSUPPORTED = 5  /* tensor index structure outside the supported set (see sp_tensor_desc) */
+} sp_status;
+
+/* Per-tensor index layout: the paper's d(u^mu) made explicit.
+ * Stored components are the canonical multi-indices in row-major order over the indices, a
+ * symmetric pair stored as its upper triangle; component c lives in state field `field[c]`.
+ * A 4-dimensional index runs (t,x,y,z), its t value is a spin-0 spectator (reading Q17); a
+ * 3-dimensional index runs (x,y,z).
+ * Supported: rank 0; rank 1; rank 2 with sym = (0,1) and equal dims; rank 3 with sym = (1,2) and
+ * equal dims on the pair (any first-index dim).  Anything else: SP_ERR_UNSUPPORTED. */
+typedef struct {
+    int rank;         /* 0..3 */
+    int index_dim[3]; /* per index: 4 = spacetime (t,x,y,z), 3 = spatial (x,y,z); unused entries ignored */
+    int sym_first;    /* indices of the one symmetric pair, or -1, -1 */
+    int sym_second;
+    const int *field; /* HOST pointer, length = number of stored components */
+} sp_tensor_desc;
+
+/* Create the shell descriptor (host only, no CUDA call).  PAPER.md:55-78 (eq. 2-5).
+ * L = highest spherical-harmonic degree KEPT by the filter, 0 <= L <= Ntheta-1 (the paper's
+ * n_f = Ntheta-1-L top degrees are removed). */
+sp_status sp_shell_create(int Nr, int Ntheta, int Nphi, double r_in, double r_out, int L, sp_shell **out);
+sp_status sp_shell_destroy(sp_shell *shell);
+
+/* Build all matrices on the host in extended precision and upload them once (PAPER.md:114, 174, 180,
+ * 215, 289, 374): CD^ (eq. 9), FD for 2 Ntheta and Nphi (eq. 8), the real Fourier analysis/synthesis
+ * matrices (eq. 23-24, with B_jm = sin, reading Q1), and F^n_m = P f P^+ (eq. 48, 49, 62) for
+ * n = -3..3, m = 0..L, built by the paper's own route: the n-recursion (42)-(44) (evaluated in
+ * binary128) and the SVD pseudo-inverse.  Synchronous.  Without a CUDA device the host matrices are
+ * still built (sp_get_matrix then works, so the host logic can be tested) but the call returns
+ * SP_ERR_CUDA and every hot call keeps returning SP_ERR_NOT_BUILT. */
+sp_status sp_build_matrices(sp_shell *shell);
+
+/* Workspace sizes in bytes for nfields fields (filter: nfields = total stored components of the
+ * tensors passed).  Any pointer may be NULL. */
+sp_status sp_workspace_bytes(const sp_shell *shell, int nfields, size_t *grad, size_t *filter, size_t *wave);
+
+/* Cartesian gradient of nfields fields (eq. 6; 98-112 eq. 7-9; 142-166 eq. 13-19; 72).
+ * u_dev: [nfields] state-shaped.  du_dev: [3][nfields] state-shaped = d/dx, d/dy, d/dz of every field
+ * (du_dev[(c*nfields + mu)*Npts + point]).  du_dev must not overlap u_dev. */
+sp_status sp_cartesian_gradient(const sp_shell *shell, const double *u_dev, int nfields, double *du_dev,
+                                void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Yn tensor filter (eq. 51-56, 60-62): dyad projection -> phi analysis (eq. 33) ->
+ * per-(n,m) theta matrix (eq. 62) -> phi synthesis (eq. 31) -> recombination, for every radius.
+ * u_dev, out_dev: [nfields] state-shaped; out_dev may equal u_dev.  Fields belonging to no tensor
+ * are copied through unchanged.  A field may belong to at most one tensor. */
+sp_status sp_tensor_filter(const sp_shell *shell, const double *u_dev, double *out_dev, int nfields,
+                           const sp_tensor_desc *tensors, int ntensors,
+                           void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* First-order scalar wave RHS with characteristic boundaries (BASELINE.json config 5; W1-W3):
+ * u = (psi, Pi, Phi_x, Phi_y, Phi_z);  d_t psi = -Pi, d_t Pi = -d_i Phi_i, d_t Phi_i = -d_i Pi; on the
+ * shells k = 0 and k = Nr-1 the incoming characteristic field is frozen (A.16). */
+sp_status sp_rhs_first_order_wave(const sp_shell *shell, const double *u_dev, double *dudt_dev,
+                                  void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* y <- a*x + b*y over n doubles (the RK4 combination steps of config 5). */
+sp_status sp_axpby(double a, const double *x_dev, double b, double *y_dev, size_t n, void *cuda_stream);
+
+/* Copy one host-built matrix out (for tests).  which: 0 = CD^ (Nr x Nr), 1 = FD_{2Ntheta} upper half
+ * (Ntheta x 2Ntheta), 2 = FD_{Nphi} (Nphi x Nphi), 3 = Fourier analysis rows (2L+1 x Nphi; row 0 = a_0,
+ * row 2m-1 = a_m, row 2m = b_m), 4 = Fourier synthesis (Nphi x 2L+1, same column order),
+ * 5 = F^n_m (Ntheta x Ntheta; n in -3..3, m in 0..L).  Row-major into host_out (may be NULL to
+ * query the shape). */
+sp_status sp_get_matrix(const sp_shell *shell, int which, int n, int m, double *host_out, int *rows, int *cols);
+
+/* Measure the FP64 issue peak of this device with a register-only DMMA (mode 0) or DFMA (mode 1)
+ * loop; returns TFLOP/s.  Used by bench.py as the live denominator of the FP64 roofline. */
+sp_status sp_probe_fp64_peak(int mode, double *tflops_out);
+
+const char *sp_status_string(sp_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPSHELL_H */

@@ -1,0 +1,111 @@
+// Cartesian gradient (eq. 6; 142-166 eq. 13-19; 72 double cover).
+//
+//   sp_cartesian_gradient = k_gemm_cols<CIRC>  (d/dphi of every field, eq. 18 without transposes -> workspace)
+//                         + k_grad_rtheta      (d/dr, d/dtheta on (r,theta) planes in shared memory, then the
+//                                               chain rule (eq. 6) with d/dphi read back, writing d/dx, d/dy, d/dz)
+#pragma once
+#include "sp_device.cuh"
+
+struct GradParams {
+    int Nr, Nt, Np, PU, Nr8, Nr4, Nt8;
+    const double *cd;       // [Nr8][PU]
+    const double *g2;       // [2Nt]
+    const double *inv_r, *sin_t, *cos_t, *inv_sin_t, *sin_p, *cos_p;
+    const double *u;        // [nf] state
+    const double *dphi;     // [nf] state (workspace)
+    double *du;             // [3][nf] state
+    int nf;
+};
+
+// One CTA per (field mu, j < Nt): owns the antipodal pair of (r,theta) planes j and j+Nt
+// (f(theta,phi) = f(2pi-theta, pi+phi)), so the double cover never touches memory.
+// Shared memory: P[2][Nt8][PU] planes (row i, column k, zero padded), CDs[Nr8][PU], g2s[2Nt].
+// Warp task = (plane, i-tile, group of KT k-tiles):
+//   d/dtheta: C[i][k]  = sum_ii g2[(i-ii) mod 2Nt] * u_ext[ii][k]     A = circulant table, B = planes
+//   d/dr    : C[i][k'] = sum_kk u[i][kk] * CD[k'][kk]                 A = plane rows,      B = CD^T
+// Both leave the same C fragment (i = i0+g, k = k0+2t,+1), so the chain rule is lane-local.
+template <int KT>
+__global__ void __launch_bounds__(512) k_grad_rtheta(GradParams p) {
+    extern __shared__ double sm[];
+    const int Nr = p.Nr, Nt = p.Nt, Np = p.Np, PU = p.PU;
+    double *P0 = sm, *P1 = sm + (size_t)p.Nt8 * PU, *CDs = P1 + (size_t)p.Nt8 * PU, *g2s = CDs + (size_t)p.Nr8 * PU;
+    const int j = blockIdx.x, mu = blockIdx.y;
+    const size_t npts = (size_t)Nr * Nt * Np, plane = (size_t)Nr * Nt;
+    const double *u0 = p.u + mu * npts + (size_t)j * plane, *u1 = u0 + (size_t)Nt * plane;
+
+    for (int q = threadIdx.x; q < 2 * p.Nt8 * PU; q += blockDim.x) sm[q] = 0.0;
+    for (int q = threadIdx.x; q < p.Nr8 * PU; q += blockDim.x) CDs[q] = p.cd[q];
+    for (int q = threadIdx.x; q < 2 * Nt; q += blockDim.x) g2s[q] = p.g2[q];
+    __syncthreads();
+    for (int q = threadIdx.x; q < Nt * Nr; q += blockDim.x) {
+        const int i = q / Nr, k = q - i * Nr;
+        P0[i * PU + k] = u0[q];
+        P1[i * PU + k] = u1[q];
+    }
+    __syncthreads();
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int itiles = p.Nt8 >> 3, ktiles = p.Nr8 >> 3, kgroups = (ktiles + KT - 1) / KT;
+    const int ntasks = 2 * itiles * kgroups;
+    const int n2 = 2 * Nt;
+    for (int task = warp; task < ntasks; task += nwarps) {
+        const int pl = task / (itiles * kgroups);
+        const int rem = task - pl * itiles * kgroups;
+        const int it = rem / kgroups, kg = rem - it * kgroups;
+        const double *Pown = pl ? P1 : P0, *Poth = pl ? P0 : P1;
+        const int i0 = it * 8, kt0 = kg * KT;
+        double at[KT][2], ar[KT][2];
+#pragma unroll
+        for (int q = 0; q < KT; q++) at[q][0] = at[q][1] = ar[q][0] = ar[q][1] = 0.0;
+        // ---- d/dtheta: K = 2Nt over the extended latitude index ii
+        const int irow = i0 + g;
+        for (int ks = 0; ks < (n2 + 3) / 4; ks++) {
+            const int ii = ks * 4 + t;
+            int d = irow - ii;
+            d += (d < 0) ? n2 : 0;
+            const double af = (ii < n2 && irow < Nt) ? g2s[d] : 0.0;
+            const int iic = ii < n2 ? ii : n2 - 1;
+            const double *rowp = (iic < Nt) ? (Pown + iic * PU) : (Poth + (n2 - 1 - iic) * PU);
+#pragma unroll
+            for (int q = 0; q < KT; q++) {
+                const int kc = (kt0 + q) * 8 + g;
+                const double bf = (kt0 + q < ktiles) ? rowp[kc] : 0.0;
+                dmma(at[q][0], at[q][1], af, bf);
+            }
+        }
+        // ---- d/dr: K = Nr over kk;  A = u[i0+g][kk], B[kk][k'] = CD[k'][kk]
+        for (int ks = 0; ks < p.Nr4 / 4; ks++) {
+            const int kk = ks * 4 + t;
+            const double af = Pown[irow * PU + kk];
+#pragma unroll
+            for (int q = 0; q < KT; q++) {
+                const int kp = (kt0 + q) * 8 + g;
+                const double bf = (kt0 + q < ktiles) ? CDs[kp * PU + kk] : 0.0;
+                dmma(ar[q][0], ar[q][1], af, bf);
+            }
+        }
+        // ---- chain rule (eq. 6), lane-local
+        if (irow < Nt) {
+            const int jj = pl ? j + Nt : j;
+            const double st = p.sin_t[irow], ct = p.cos_t[irow], ist = p.inv_sin_t[irow];
+            const double sp = p.sin_p[jj], cp = p.cos_p[jj];
+            const size_t base = (size_t)mu * npts + (size_t)jj * plane + (size_t)irow * Nr;
+            const size_t fs = (size_t)p.nf * npts;
+#pragma unroll
+            for (int q = 0; q < KT; q++) {
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    const int k = (kt0 + q) * 8 + 2 * t + e;
+                    if (k < Nr) {
+                        const double ir = p.inv_r[k];
+                        const double a = ar[q][e], b = at[q][e] * ir, c = p.dphi[base + k] * ir * ist;
+                        p.du[base + k] = st * cp * a + ct * cp * b - sp * c;
+                        p.du[fs + base + k] = st * sp * a + ct * sp * b + cp * c;
+                        p.du[2 * fs + base + k] = ct * a - st * b;
+                    }
+                }
+            }
+        }
+    }
+}

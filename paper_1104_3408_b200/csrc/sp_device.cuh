@@ -1,0 +1,39 @@
+// Shell object and device-side helpers shared by the kernels of libspshell.
+#pragma once
+#include "../../include/spshell.h"
+#include "sp_internal.h"
+
+#include <cuda_runtime.h>
+
+struct sp_shell {
+    int Nr, Nt, Np, L;
+    double rin, rout;
+    int Nr8, Nr4, Nt8, Nt4, MC, MC4, MC8, J8, PU;
+    size_t npts;
+    bool built, host_built;
+    SpHostMatrices *host = nullptr;
+    // device-resident tables (owned)
+    double *d_cd = nullptr;        // CD^ [Nr8][PU], zero padded                       (eq. 9)
+    double *d_g2 = nullptr;        // FD_{2Nt} circulant generator [2Nt]               (eq. 8)
+    double *d_g3 = nullptr;        // FD_{Np}  circulant generator [Np]
+    double *d_an = nullptr;        // Fourier analysis  [MC8][Np], zero padded rows    (eq. 24)
+    double *d_sy = nullptr;        // Fourier synthesis [J8][MC4], zero padded         (eq. 23)
+    double *d_F = nullptr;         // F^n_m [7][L+1][Nt8][Nt4], zero padded            (eq. 62)
+    double *d_inv_r = nullptr, *d_sin_t = nullptr, *d_cos_t = nullptr, *d_inv_sin_t = nullptr, *d_sin_p = nullptr,
+           *d_cos_p = nullptr;     // Jacobian / triad factors                          (eq. 6, 51)
+};
+
+sp_status sp_configure_kernels(sp_shell *s);
+
+// ---------------------------------------------------------------------------------------------
+// FP64 tensor-core tile: D(8x8) += A(8x4) * B(4x8), SASS DMMA.8x8x4 (the only native FP64 MMA shape
+// on sm_100a).  Fragment ownership for lane l, g = l>>2, t = l&3:
+//     A[g][t]            (row-major 8x4)
+//     B[t][g]            (4x8, "col" operand)
+//     C[g][2t], C[g][2t+1]
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}

@@ -1,0 +1,419 @@
+// libspshell -- C ABI entry points and shell object (see include/spshell.h).
+// Kernels live in kernels_*.cuh; the host matrix construction in host_build.cpp.
+#include "../../include/spshell.h"
+#include "sp_internal.h"
+#include "sp_device.cuh"
+
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#define SP_CUDA(x)                                   \
+    do {                                             \
+        cudaError_t e_ = (x);                        \
+        if (e_ != cudaSuccess) return SP_ERR_CUDA;   \
+    } while (0)
+
+static int round_up(int a, int b) { return (a + b - 1) / b * b; }
+
+extern "C" const char *sp_status_string(sp_status s) {
+    switch (s) {
+        case SP_OK: return "SP_OK";
+        case SP_ERR_INVALID_ARG: return "SP_ERR_INVALID_ARG";
+        case SP_ERR_NOT_BUILT: return "SP_ERR_NOT_BUILT";
+        case SP_ERR_ALLOC: return "SP_ERR_ALLOC";
+        case SP_ERR_CUDA: return "SP_ERR_CUDA";
+        case SP_ERR_UNSUPPORTED: return "SP_ERR_UNSUPPORTED";
+    }
+    return "SP_ERR_?";
+}
+
+extern "C" sp_status sp_shell_create(int Nr, int Nt, int Np, double rin, double rout, int L, sp_shell **out) {
+    if (!out) return SP_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (Nr < 2 || Nt < 2 || Np != 2 * Nt) return SP_ERR_INVALID_ARG;          // eq. 5
+    if (!(rin > 0) || !(rout > rin)) return SP_ERR_INVALID_ARG;
+    if (L < 0 || L > Nt - 1) return SP_ERR_INVALID_ARG;
+    sp_shell *s = new (std::nothrow) sp_shell();
+    if (!s) return SP_ERR_ALLOC;
+    s->Nr = Nr; s->Nt = Nt; s->Np = Np; s->L = L; s->rin = rin; s->rout = rout;
+    s->Nr8 = round_up(Nr, 8); s->Nr4 = round_up(Nr, 4);
+    s->Nt8 = round_up(Nt, 8); s->Nt4 = round_up(Nt, 4);
+    s->MC = 2 * L + 1; s->MC4 = round_up(s->MC, 4); s->MC8 = round_up(s->MC, 8);
+    s->J8 = round_up(Np, 8);
+    s->PU = s->Nr8 + 4;                                                       // smem pitch == 4 (mod 8): conflict-free fragments
+    s->npts = (size_t)Nr * Nt * Np;
+    s->built = false; s->host_built = false;
+    *out = s;
+    return SP_OK;
+}
+
+static void free_dev(sp_shell *s) {
+    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
+                    &s->d_inv_sin_t, &s->d_sin_p, &s->d_cos_p};
+    for (auto q : p) {
+        if (*q) cudaFree(*q);
+        *q = nullptr;
+    }
+}
+
+extern "C" sp_status sp_shell_destroy(sp_shell *s) {
+    if (!s) return SP_ERR_INVALID_ARG;
+    free_dev(s);
+    delete s->host;
+    delete s;
+    return SP_OK;
+}
+
+static sp_status upload(double **dst, const double *src, size_t n) {
+    SP_CUDA(cudaMalloc((void **)dst, n * sizeof(double)));
+    SP_CUDA(cudaMemcpy(*dst, src, n * sizeof(double), cudaMemcpyHostToDevice));
+    return SP_OK;
+}
+
+extern "C" sp_status sp_build_matrices(sp_shell *s) {
+    if (!s) return SP_ERR_INVALID_ARG;
+    s->built = false;
+    delete s->host;
+    s->host = new (std::nothrow) SpHostMatrices();
+    if (!s->host) return SP_ERR_ALLOC;
+    SpHostMatrices &H = *s->host;
+    sp_host_build(s->Nr, s->Nt, s->Np, s->rin, s->rout, s->L, H);
+    s->host_built = true;                      // sp_get_matrix works from here on (host logic is testable)
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return SP_ERR_CUDA;   // no CPU fallback for the hot path
+    free_dev(s);
+    const int Nr = s->Nr, Nt = s->Nt, Np = s->Np, L = s->L;
+    sp_status st;
+    // CD^ padded [Nr8][PU], zeros outside
+    {
+        std::vector<double> t((size_t)s->Nr8 * s->PU, 0.0);
+        for (int i = 0; i < Nr; i++)
+            for (int j = 0; j < Nr; j++) t[(size_t)i * s->PU + j] = H.cd[(size_t)i * Nr + j];
+        if ((st = upload(&s->d_cd, t.data(), t.size())) != SP_OK) return st;
+    }
+    if ((st = upload(&s->d_g2, H.g2.data(), H.g2.size())) != SP_OK) return st;
+    if ((st = upload(&s->d_g3, H.g3.data(), H.g3.size())) != SP_OK) return st;
+    {   // analysis [MC8][Np], synthesis [J8][MC4]
+        std::vector<double> a((size_t)s->MC8 * Np, 0.0), y((size_t)s->J8 * s->MC4, 0.0);
+        for (int m = 0; m < s->MC; m++)
+            for (int j = 0; j < Np; j++) a[(size_t)m * Np + j] = H.an[(size_t)m * Np + j];
+        for (int j = 0; j < Np; j++)
+            for (int m = 0; m < s->MC; m++) y[(size_t)j * s->MC4 + m] = H.sy[(size_t)j * s->MC + m];
+        if ((st = upload(&s->d_an, a.data(), a.size())) != SP_OK) return st;
+        if ((st = upload(&s->d_sy, y.data(), y.size())) != SP_OK) return st;
+    }
+    {   // F [7][L+1][Nt8][Nt4]
+        std::vector<double> f((size_t)7 * (L + 1) * s->Nt8 * s->Nt4, 0.0);
+        for (int q = 0; q < 7 * (L + 1); q++)
+            for (int i = 0; i < Nt; i++)
+                for (int j = 0; j < Nt; j++)
+                    f[((size_t)q * s->Nt8 + i) * s->Nt4 + j] = H.F[((size_t)q * Nt + i) * Nt + j];
+        if ((st = upload(&s->d_F, f.data(), f.size())) != SP_OK) return st;
+    }
+    if ((st = upload(&s->d_inv_r, H.inv_r.data(), Nr)) != SP_OK) return st;
+    if ((st = upload(&s->d_sin_t, H.sin_t.data(), Nt)) != SP_OK) return st;
+    if ((st = upload(&s->d_cos_t, H.cos_t.data(), Nt)) != SP_OK) return st;
+    if ((st = upload(&s->d_inv_sin_t, H.inv_sin_t.data(), Nt)) != SP_OK) return st;
+    if ((st = upload(&s->d_sin_p, H.sin_p.data(), Np)) != SP_OK) return st;
+    if ((st = upload(&s->d_cos_p, H.cos_p.data(), Np)) != SP_OK) return st;
+    if ((st = sp_configure_kernels(s)) != SP_OK) return st;
+    s->built = true;
+    return SP_OK;
+}
+
+extern "C" sp_status sp_get_matrix(const sp_shell *s, int which, int n, int m, double *out, int *rows, int *cols) {
+    if (!s) return SP_ERR_INVALID_ARG;
+    if (!s->host_built) return SP_ERR_NOT_BUILT;
+    const SpHostMatrices &H = *s->host;
+    const int Nr = s->Nr, Nt = s->Nt, Np = s->Np, L = s->L, MC = s->MC;
+    int r = 0, c = 0;
+    switch (which) {
+        case 0: r = c = Nr; break;
+        case 1: r = Nt; c = 2 * Nt; break;
+        case 2: r = c = Np; break;
+        case 3: r = MC; c = Np; break;
+        case 4: r = Np; c = MC; break;
+        case 5:
+            if (n < -3 || n > 3 || m < 0 || m > L) return SP_ERR_INVALID_ARG;
+            r = c = Nt; break;
+        default: return SP_ERR_INVALID_ARG;
+    }
+    if (rows) *rows = r;
+    if (cols) *cols = c;
+    if (!out) return SP_OK;
+    switch (which) {
+        case 0: memcpy(out, H.cd.data(), sizeof(double) * r * c); break;
+        case 1:
+            for (int i = 0; i < r; i++)
+                for (int j = 0; j < c; j++) out[(size_t)i * c + j] = H.g2[((i - j) % c + c) % c];
+            break;
+        case 2:
+            for (int i = 0; i < r; i++)
+                for (int j = 0; j < c; j++) out[(size_t)i * c + j] = H.g3[((i - j) % c + c) % c];
+            break;
+        case 3: memcpy(out, H.an.data(), sizeof(double) * r * c); break;
+        case 4: memcpy(out, H.sy.data(), sizeof(double) * r * c); break;
+        case 5: memcpy(out, &H.F[((size_t)(n + 3) * (L + 1) + m) * Nt * Nt], sizeof(double) * r * c); break;
+    }
+    return SP_OK;
+}
+
+// =================================================================================================
+// Hot calls
+// =================================================================================================
+#include "kernels_gemm.cuh"
+#include "kernels_grad.cuh"
+#include "kernels_filter.cuh"
+#include "kernels_wave.cuh"
+
+static size_t grad_smem_bytes(const sp_shell *s) {
+    return ((size_t)2 * s->Nt8 * s->PU + (size_t)s->Nr8 * s->PU + 2 * s->Nt) * sizeof(double);
+}
+
+sp_status sp_configure_kernels(sp_shell *s) {
+    size_t sm = grad_smem_bytes(s);
+    if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;       // (r,theta) plane pair must fit one SM's shared memory
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    return SP_OK;
+}
+
+extern "C" sp_status sp_workspace_bytes(const sp_shell *s, int nfields, size_t *grad, size_t *filter, size_t *wave) {
+    if (!s || nfields < 0) return SP_ERR_INVALID_ARG;
+    const size_t vec = (size_t)s->Nt * s->Nr;
+    if (grad) *grad = (size_t)nfields * s->npts * sizeof(double);
+    if (filter) *filter = (size_t)nfields * (s->npts + 2 * (size_t)s->MC4 * vec) * sizeof(double);
+    if (wave) *wave = (size_t)(4 + 12) * s->npts * sizeof(double);
+    return SP_OK;
+}
+
+extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, int nf, double *du, void *ws, size_t wsb,
+                                           void *stream) {
+    if (!s || !u || !du || nf < 0) return SP_ERR_INVALID_ARG;
+    if (!s->built) return SP_ERR_NOT_BUILT;
+    if (nf == 0) return SP_OK;
+    if (!ws || wsb < (size_t)nf * s->npts * sizeof(double)) return SP_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Nr = s->Nr, Nt = s->Nt, Np = s->Np;
+    const long plane = (long)Nr * Nt;
+    double *dphi = (double *)ws;
+    // d/dphi: FD_{Np} (circulant) over j, stride Nr*Nt; every field is one batch          (eq. 8, 18)
+    sp_status e = launch_gemm_cols<true>(s->d_g3, Np, Np, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts,
+                                         (int)plane, nf, st);
+    if (e != SP_OK) return e;
+    GradParams p;
+    p.Nr = Nr; p.Nt = Nt; p.Np = Np; p.PU = s->PU; p.Nr8 = s->Nr8; p.Nr4 = s->Nr4; p.Nt8 = s->Nt8;
+    p.cd = s->d_cd; p.g2 = s->d_g2;
+    p.inv_r = s->d_inv_r; p.sin_t = s->d_sin_t; p.cos_t = s->d_cos_t; p.inv_sin_t = s->d_inv_sin_t;
+    p.sin_p = s->d_sin_p; p.cos_p = s->d_cos_p;
+    p.u = u; p.dphi = dphi; p.du = du; p.nf = nf;
+    const int itiles = s->Nt8 / 8, ktiles = s->Nr8 / 8;
+    const size_t sm = grad_smem_bytes(s);
+    dim3 grid(Nt, nf);
+    if (ktiles <= 3 || ktiles == 6 || ktiles == 9) {
+        int ntasks = 2 * itiles * ((ktiles + 2) / 3);
+        int nw = ntasks < 16 ? ntasks : 16;
+        k_grad_rtheta<3><<<grid, nw * 32, sm, st>>>(p);
+    } else {
+        int ntasks = 2 * itiles * ((ktiles + 4) / 5);
+        int nw = ntasks < 16 ? ntasks : 16;
+        k_grad_rtheta<5><<<grid, nw * 32, sm, st>>>(p);
+    }
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
+// ---- tensor classification -------------------------------------------------------------------
+static int classify(const sp_tensor_desc &d) {
+    auto okdim = [](int x) { return x == 3 || x == 4; };
+    switch (d.rank) {
+        case 0: return TT_SCALAR;
+        case 1:
+            if (!okdim(d.index_dim[0])) return -1;
+            return d.index_dim[0] == 3 ? TT_VEC3 : TT_VEC4;
+        case 2:
+            if (!okdim(d.index_dim[0]) || d.index_dim[0] != d.index_dim[1]) return -2;
+            if (!((d.sym_first == 0 && d.sym_second == 1) || (d.sym_first == 1 && d.sym_second == 0))) return -2;
+            return d.index_dim[0] == 3 ? TT_SYM3 : TT_SYM4;
+        case 3:
+            if (!okdim(d.index_dim[0]) || !okdim(d.index_dim[1]) || d.index_dim[1] != d.index_dim[2]) return -2;
+            if (!((d.sym_first == 1 && d.sym_second == 2) || (d.sym_first == 2 && d.sym_second == 1))) return -2;
+            if (d.index_dim[0] == 3) return d.index_dim[1] == 3 ? TT_R3_3_3 : TT_R3_3_4;
+            return d.index_dim[1] == 3 ? TT_R3_4_3 : TT_R3_4_4;
+    }
+    return -1;
+}
+static int tt_ncomp(int tt) {
+    static const int n[TT_COUNT] = {1, 3, 4, 6, 10, 18, 30, 24, 40};
+    return n[tt];
+}
+// spin-weight components of a tensor type in dof order: appends (dof, n, cplx)
+static void tt_components(int tt, int dof0, std::vector<ThetaComp> &out) {
+    int d = dof0;
+    auto real = [&]() { out.push_back({d, 0, 0}); d += 1; };
+    auto cplx = [&](int n) { out.push_back({d, n, 1}); d += 2; };
+    auto sym = [&](int D, int shift, bool only_complex, bool as_complex_real) {
+        int nreal = (D == 4) ? 4 : 2;
+        if (!only_complex)
+            for (int q = 0; q < nreal; q++) { if (as_complex_real) cplx(shift); else real(); }
+        if (as_complex_real && !only_complex) return;
+        if (D == 4) cplx(1 + shift);
+        cplx(1 + shift);
+        cplx(2 + shift);
+    };
+    switch (tt) {
+        case TT_SCALAR: real(); break;
+        case TT_VEC3: real(); cplx(1); break;
+        case TT_VEC4: real(); real(); cplx(1); break;
+        case TT_SYM3: sym(3, 0, false, false); break;
+        case TT_SYM4: sym(4, 0, false, false); break;
+        default: {
+            const int D1 = (tt == TT_R3_4_3 || tt == TT_R3_4_4) ? 4 : 3;
+            const int D2 = (tt == TT_R3_3_4 || tt == TT_R3_4_4) ? 4 : 3;
+            if (D1 == 4) sym(D2, 0, false, false);       // first index t
+            sym(D2, 0, false, false);                     // first index r^
+            sym(D2, 1, false, true);                      // [m; real entries]: complex, n = +1
+            sym(D2, 1, true, false);                      // [m; complex entries]: n_e + 1
+            sym(D2, -1, true, false);                     // [mbar; complex entries]: n_e - 1
+        }
+    }
+}
+
+template <bool INV>
+static void launch_pointwise(int tt, const TensorArgs &ta, const sp_shell *s, const double *src, double *dst, cudaStream_t st) {
+    const int T = 128;
+    const unsigned nb = (unsigned)((s->npts + T - 1) / T);
+#define SP_PW(TTV)                                                                                                        \
+    case TTV:                                                                                                             \
+        k_pointwise<TTV, INV><<<nb, T, 0, st>>>(ta, s->Nr, s->Nt, s->npts, s->d_sin_t, s->d_cos_t, s->d_sin_p, s->d_cos_p, \
+                                                src, dst);                                                                \
+        break;
+    switch (tt) {
+        SP_PW(TT_SCALAR) SP_PW(TT_VEC3) SP_PW(TT_VEC4) SP_PW(TT_SYM3) SP_PW(TT_SYM4) SP_PW(TT_R3_3_3) SP_PW(TT_R3_3_4)
+        SP_PW(TT_R3_4_3) SP_PW(TT_R3_4_4)
+    }
+#undef SP_PW
+}
+
+extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double *out, int nfields, const sp_tensor_desc *tens,
+                                      int ntens, void *ws, size_t wsb, void *stream) {
+    if (!s || !u || !out || nfields < 0 || ntens < 0 || (ntens > 0 && !tens)) return SP_ERR_INVALID_ARG;
+    if (!s->built) return SP_ERR_NOT_BUILT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Nr = s->Nr, Nt = s->Nt, Np = s->Np;
+    const size_t npts = s->npts, vec = (size_t)Nt * Nr;
+    // ---- validate, classify, build the component list
+    std::vector<int> owner(nfields, -1), types(ntens);
+    std::vector<TensorArgs> targs(ntens);
+    std::vector<ThetaComp> comps;
+    int ndof = 0;
+    for (int t = 0; t < ntens; t++) {
+        const sp_tensor_desc &d = tens[t];
+        if (d.rank < 0 || d.rank > 3 || !d.field) return SP_ERR_INVALID_ARG;
+        int tt = classify(d);
+        if (tt == -1) return SP_ERR_INVALID_ARG;
+        if (tt < 0) return SP_ERR_UNSUPPORTED;
+        types[t] = tt;
+        TensorArgs &a = targs[t];
+        a.ncomp = tt_ncomp(tt);
+        a.dof0 = ndof;
+        for (int c = 0; c < a.ncomp; c++) {
+            int f = d.field[c];
+            if (f < 0 || f >= nfields || owner[f] >= 0) return SP_ERR_INVALID_ARG;
+            owner[f] = t;
+            a.field[c] = f;
+        }
+        tt_components(tt, ndof, comps);
+        ndof += a.ncomp;
+    }
+    if (out != u)
+        for (int f = 0; f < nfields; f++)
+            if (owner[f] < 0) SP_CUDA(cudaMemcpyAsync(out + f * npts, u + f * npts, npts * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    if (ndof == 0) return SP_OK;
+    const size_t need = (size_t)ndof * (npts + 2 * (size_t)s->MC4 * vec) * sizeof(double);
+    if (!ws || wsb < need) return SP_ERR_INVALID_ARG;
+    double *dofs = (double *)ws, *coef1 = dofs + (size_t)ndof * npts, *coef2 = coef1 + (size_t)ndof * s->MC4 * vec;
+    // ---- F1: dyad projection
+    for (int t = 0; t < ntens; t++) launch_pointwise<false>(types[t], targs[t], s, u, dofs, st);
+    // ---- F2: phi analysis (eq. 33)
+    sp_status e = launch_gemm_cols<false>(s->d_an, Np, s->MC, Np, dofs, (long)vec, (long)npts, coef1, (long)vec,
+                                          (long)(s->MC4 * vec), (int)vec, ndof, st);
+    if (e != SP_OK) return e;
+    // ---- F3: per-(n,m) theta matrices (eq. 62)
+    {
+        const int nwarps = (Nr + 3) / 4, mtiles = s->Nt8 / 8;
+        for (size_t c0 = 0; c0 < comps.size(); c0 += SP_THETA_BATCH) {
+            ThetaBatch b;
+            int nb = (int)std::min<size_t>(SP_THETA_BATCH, comps.size() - c0);
+            for (int q = 0; q < nb; q++) b.c[q] = comps[c0 + q];
+            if (nwarps > 20) return SP_ERR_UNSUPPORTED;
+            if (mtiles % 3 == 0) {
+                dim3 grid(s->L + 1, nb, mtiles / 3);
+                k_theta<3><<<grid, nwarps * 32, 0, st>>>(b, s->d_F, s->L, Nt, s->Nt8, s->Nt4, Nr, s->MC4, coef1, coef2);
+            } else {
+                dim3 grid(s->L + 1, nb, (mtiles + 3) / 4);
+                k_theta<4><<<grid, nwarps * 32, 0, st>>>(b, s->d_F, s->L, Nt, s->Nt8, s->Nt4, Nr, s->MC4, coef1, coef2);
+            }
+        }
+        if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
+    }
+    // ---- F4: phi synthesis (eq. 31)
+    e = launch_gemm_cols<false>(s->d_sy, s->MC4, Np, s->MC, coef2, (long)vec, (long)(s->MC4 * vec), dofs, (long)vec, (long)npts,
+                                (int)vec, ndof, st);
+    if (e != SP_OK) return e;
+    // ---- F5: recombination
+    for (int t = 0; t < ntens; t++) launch_pointwise<true>(types[t], targs[t], s, dofs, out, st);
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
+extern "C" sp_status sp_rhs_first_order_wave(const sp_shell *s, const double *u, double *dudt, void *ws, size_t wsb, void *stream) {
+    if (!s || !u || !dudt) return SP_ERR_INVALID_ARG;
+    if (!s->built) return SP_ERR_NOT_BUILT;
+    const size_t npts = s->npts;
+    if (!ws || wsb < 16 * npts * sizeof(double)) return SP_ERR_INVALID_ARG;
+    double *gws = (double *)ws, *dg = gws + 4 * npts;
+    sp_status e = sp_cartesian_gradient(s, u + npts, 4, dg, gws, 4 * npts * sizeof(double), stream);
+    if (e != SP_OK) return e;
+    const int T = 256;
+    k_wave_rhs<<<(unsigned)((npts + T - 1) / T), T, 0, (cudaStream_t)stream>>>(s->Nr, s->Nt, npts, s->d_sin_t, s->d_cos_t, s->d_sin_p,
+                                                                              s->d_cos_p, u, dg, dudt);
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
+extern "C" sp_status sp_axpby(double a, const double *x, double b, double *y, size_t n, void *stream) {
+    if (!x || !y) return SP_ERR_INVALID_ARG;
+    if (n == 0) return SP_OK;
+    size_t nb = (n + 255) / 256;
+    if (nb > 148 * 16) nb = 148 * 16;
+    k_axpby<<<(unsigned)nb, 256, 0, (cudaStream_t)stream>>>(a, x, b, y, n);
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
+extern "C" sp_status sp_probe_fp64_peak(int mode, double *tflops) {
+    if (!tflops || mode < 0 || mode > 1) return SP_ERR_INVALID_ARG;
+    cudaDeviceProp prop;
+    SP_CUDA(cudaGetDeviceProperties(&prop, 0));
+    const int grid = prop.multiProcessorCount * 2, thr = 512, iters = 20000;
+    double *buf = nullptr;
+    SP_CUDA(cudaMalloc((void **)&buf, sizeof(double) * grid * thr));
+    cudaEvent_t e0, e1;
+    SP_CUDA(cudaEventCreate(&e0));
+    SP_CUDA(cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 6; rep++) {
+        cudaEventRecord(e0);
+        if (mode == 0) k_probe_dmma<<<grid, thr>>>(buf, iters, 1.0000001, 1e-9);
+        else k_probe_dfma<<<grid, thr>>>(buf, iters, 1.0000001, 1e-9);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(buf); return SP_ERR_CUDA; }
+        float ms;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    const double flops = (mode == 0) ? 2.0 * 256 * 8 * iters * (double)grid * (thr / 32) : 2.0 * 16 * iters * (double)grid * thr;
+    *tflops = flops / (best * 1e-3) * 1e-12;
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(buf);
+    return SP_OK;
+}

@@ -47,13 +47,13 @@ def _synthesise(coef, T, P, phi, decay_l, decay_q):
     c = coef * wq[:, None, None] * wl[None, :, None]
     R = T[:, :nq] @ c.reshape(nq, -1)                                      # [k, (l, m)]
     R = R.reshape(Nr, lmax + 1, 2 * lmax + 1)
-    out = np.zeros((phi.size, Nt, Nr))
+    X = np.empty((2 * lmax + 1, Nt, Nr))
+    trig = np.empty((phi.size, 2 * lmax + 1))
     for m in range(-lmax, lmax + 1):
         am = abs(m)
-        X = np.einsum("kl,li->ik", R[:, am:, m + lmax], P[am:, am, :])    # [i, k]
-        trig = np.cos(am * phi) if m >= 0 else np.sin(am * phi)
-        out += trig[:, None, None] * X[None, :, :]
-    return out
+        X[m + lmax] = (R[:, am:, m + lmax] @ P[am:, am, :]).T              # [i, k]
+        trig[:, m + lmax] = np.cos(am * phi) if m >= 0 else np.sin(am * phi)
+    return (trig @ X.reshape(2 * lmax + 1, Nt * Nr)).reshape(phi.size, Nt, Nr)
 
 
 def make_state(cfg, decay=True, lmax=None, nfields=None, seed=None):

@@ -1,0 +1,177 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerance: 1e-12 relative, max-norm over each field (north_star)."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _shell(cfg):
+    from paper_1104_3408_b200 import Shell
+    return Shell(cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["rmin"], cfg["rmax"], cfg["L"])
+
+
+def _rel(a, b):
+    """worst field of max|a-b| / max|b| (fields = leading axes, last three axes are the grid)."""
+    a = a.reshape(-1, a.shape[-3] * a.shape[-2] * a.shape[-1])
+    b = b.reshape(a.shape)
+    den = np.max(np.abs(b), axis=1)
+    den[den == 0] = 1.0
+    return float(np.max(np.max(np.abs(a - b), axis=1) / den))
+
+
+def _grad_gpu(sh, u):
+    torch = _torch()
+    return sh.cartesian_gradient(torch.from_numpy(u).cuda()).cpu().numpy()
+
+
+def _filt_gpu(sh, u, tensors):
+    torch = _torch()
+    return sh.tensor_filter(torch.from_numpy(u).cuda(), tensors).cpu().numpy()
+
+
+@pytest.mark.parametrize("cid,white", [(1, False), (2, False), (2, True), (3, False)])
+def test_gradient_full(cid, white):
+    cfg = synth.config(cid)
+    u = synth.white_state(cfg) if white else synth.make_state(cfg)
+    nf = u.shape[0] if cid < 3 else 10                      # config 3: 10 of the 50 fields in full
+    u = np.ascontiguousarray(u[:nf])
+    got = _grad_gpu(_shell(cfg), u)
+    want = oracle.gradient(u, cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["rmin"], cfg["rmax"])
+    assert _rel(got, want) < TOL
+
+
+@pytest.mark.parametrize("cid", [3, 4, 5])
+def test_gradient_sampled_full_size(cid):
+    """Full-size launch (the bench configuration), oracle on 3000 sampled outputs + field max-norms."""
+    cfg = synth.config(cid)
+    u = synth.make_state(cfg)
+    got = _grad_gpu(_shell(cfg), u)
+    rng = np.random.default_rng(cid)
+    ns = 3000
+    samp = np.stack([rng.integers(cfg["Nr"], size=ns), rng.integers(cfg["Nt"], size=ns), rng.integers(cfg["Np"], size=ns),
+                     rng.integers(cfg["nfields"], size=ns)], axis=1).astype(np.int32)
+    samp[:40, 0] = 0; samp[40:80, 0] = cfg["Nr"] - 1; samp[80:120, 1] = 0; samp[120:160, 1] = cfg["Nt"] - 1   # edges, poles
+    want = oracle.gradient_at(u, cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["rmin"], cfg["rmax"], samp)
+    fmax = np.max(np.abs(got.reshape(3, cfg["nfields"], -1)), axis=2)        # [3, nf]
+    for s, (k, i, j, mu) in enumerate(samp):
+        g = got[:, mu, j, i, k]
+        assert np.all(np.abs(g - want[s]) <= TOL * fmax[:, mu]), (s, g, want[s])
+
+
+@pytest.mark.parametrize("cid,white", [(1, False), (2, False), (2, True)])
+def test_filter_full(cid, white):
+    cfg = synth.config(cid)
+    u = synth.white_state(cfg) if white else synth.make_state(cfg)
+    got = _filt_gpu(_shell(cfg), u, cfg["tensors"])
+    want = oracle.tensor_filter(u, cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["L"], cfg["tensors"])
+    assert _rel(got, want) < TOL
+    if cid == 1:      # config 1's data lies inside the kept band: the filter must preserve it
+        assert _rel(got, u) < TOL
+
+
+@pytest.mark.parametrize("cid,radii,white", [(3, (0, 17), False), (3, (32,), True), (4, (40,), True), (5, (5,), False)])
+def test_filter_sampled_radii_full_size(cid, radii, white):
+    """Full-size launch; the oracle filters whole spheres at sampled radii (F is independent of r)."""
+    cfg = synth.config(cid)
+    if white:
+        u = synth.white_state(cfg)
+    else:
+        u = synth.make_state(cfg)
+    got = _filt_gpu(_shell(cfg), u, cfg["tensors"])
+    for k in radii:
+        want = oracle.tensor_filter(u, cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["L"], cfg["tensors"], ksel=k)
+        a, b = got[..., k:k + 1], want[..., k:k + 1]
+        assert _rel(a, b) < TOL, (cid, k)
+
+
+TYPES = [
+    {"rank": 0, "dims": (), "sym": (-1, -1)},
+    {"rank": 1, "dims": (3,), "sym": (-1, -1)},
+    {"rank": 1, "dims": (4,), "sym": (-1, -1)},
+    {"rank": 2, "dims": (3, 3), "sym": (0, 1)},
+    {"rank": 2, "dims": (4, 4), "sym": (0, 1)},
+    {"rank": 3, "dims": (3, 3, 3), "sym": (1, 2)},
+    {"rank": 3, "dims": (3, 4, 4), "sym": (1, 2)},
+    {"rank": 3, "dims": (4, 3, 3), "sym": (1, 2)},
+    {"rank": 3, "dims": (4, 4, 4), "sym": (1, 2)},
+]
+
+
+@pytest.mark.parametrize("shape", [(5, 7, 14, 4), (9, 8, 16, 6), (6, 10, 20, 9), (12, 9, 18, 0)])
+def test_every_tensor_type_ragged_grids(shape):
+    """All supported index structures on grids that are not multiples of the 8x8x4 tile (odd Ntheta,
+    even Nr, L = 0 and L = Ntheta-1), white-noise data, scattered field order, pass-through fields."""
+    from paper_1104_3408_b200 import Shell
+    Nr, Nt, Np, L = shape
+    rng = np.random.default_rng(Nr * 100 + Nt)
+    tensors, nf = [], 0
+    for t in TYPES:
+        nc = synth.tensor_ncomp(t)
+        tensors.append(dict(t, fields=list(range(nf, nf + nc))))
+        nf += nc + 1                                           # leave a gap field that no tensor owns
+    perm = rng.permutation(nf)
+    for t in tensors:
+        t["fields"] = [int(perm[f]) for f in t["fields"]]
+    u = rng.standard_normal((nf, Np, Nt, Nr))
+    sh = Shell(Nr, Nt, Np, 1.3, 4.1, L)
+    got = _filt_gpu(sh, u, tensors)
+    want = oracle.tensor_filter(u, Nr, Nt, Np, L, tensors)
+    assert _rel(got, want) < TOL
+    owned = {f for t in tensors for f in t["fields"]}
+    for f in range(nf):
+        if f not in owned:
+            assert np.array_equal(got[f], u[f])
+    g = _grad_gpu(sh, u)
+    assert _rel(g, oracle.gradient(u, Nr, Nt, Np, 1.3, 4.1)) < TOL
+
+
+def test_filter_invariants_and_edge_cases():
+    torch = _torch()
+    from paper_1104_3408_b200 import Shell, SpError
+    cfg = synth.config(2)
+    sh = _shell(cfg)
+    u = torch.from_numpy(synth.white_state(cfg)).cuda()
+    f1 = sh.tensor_filter(u, cfg["tensors"])
+    f2 = sh.tensor_filter(f1, cfg["tensors"])
+    assert _rel(f2.cpu().numpy(), f1.cpu().numpy()) < TOL          # idempotent
+    f1b = sh.tensor_filter(u, cfg["tensors"])
+    assert torch.equal(f1, f1b)                                    # deterministic, bit for bit
+    v = u.clone()
+    sh.tensor_filter(v, cfg["tensors"], out=v)                     # in place
+    assert torch.equal(v, f1)
+    g1 = sh.cartesian_gradient(u); g2 = sh.cartesian_gradient(u)
+    assert torch.equal(g1, g2)
+    # empty inputs
+    e = torch.empty((0, cfg["Np"], cfg["Nt"], cfg["Nr"]), dtype=torch.float64, device="cuda")
+    assert sh.cartesian_gradient(e).numel() == 0
+    assert torch.equal(sh.tensor_filter(u, []), u)                 # no tensors: copy through
+    # errors: a field in two tensors; unsupported structure; short workspace
+    bad = [dict(cfg["tensors"][0]), dict(cfg["tensors"][0])]
+    with pytest.raises(SpError):
+        sh.tensor_filter(u, bad)
+    with pytest.raises(SpError):
+        sh.tensor_filter(u, [{"rank": 2, "dims": (3, 3), "sym": (-1, -1), "fields": list(range(9))}])
+    with pytest.raises(SpError):
+        sh.cartesian_gradient(u, workspace=torch.empty(8, dtype=torch.float64, device="cuda"))
+
+
+def test_gradient_exact_polynomial_on_gpu():
+    """Invariant that needs no oracle: exact Cartesian gradient of a polynomial in x, y, z."""
+    cfg = synth.config(2)
+    r, th, ph = oracle.grid(cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["rmin"], cfg["rmax"])
+    P, T, R = np.meshgrid(ph, th, r, indexing="ij")
+    x, y, z = R * np.sin(T) * np.cos(P), R * np.sin(T) * np.sin(P), R * np.cos(T)
+    f = (x ** 3 * y - 2 * z ** 2 * x + y * z) / 100.0
+    g = _grad_gpu(_shell(cfg), f[None])
+    want = np.stack([(3 * x ** 2 * y - 2 * z ** 2) / 100, (x ** 3 + z) / 100, (-4 * z * x + y) / 100])[:, None]
+    assert _rel(g, want) < 1e-11

@@ -1,0 +1,61 @@
+"""Library host logic on the CPU: the C-ABI library loads and exports every declared symbol, argument
+validation, and the host-built matrices (the paper's recursion (42)-(44) in binary128 + Jacobi SVD)
+against the oracle's (Wigner-d l-recurrence + Householder QR) -- two independent routes."""
+import ctypes as C
+import re
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1104_3408_b200 import Shell, SpError, binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "spshell.h")).read()
+    declared = set(re.findall(r"\b(sp_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.EXPORTED_SYMBOLS)
+    L = binding.lib()
+    for s in declared:
+        assert hasattr(L, s), s
+
+
+def test_argument_validation():
+    L = binding.lib()
+    h = C.c_void_p()
+    bad = [(9, 8, 15, 1.0, 3.0, 6), (1, 8, 16, 1.0, 3.0, 6), (9, 1, 2, 1.0, 3.0, 0), (9, 8, 16, 3.0, 1.0, 6),
+           (9, 8, 16, 0.0, 1.0, 6), (9, 8, 16, 1.0, 3.0, 8), (9, 8, 16, 1.0, 3.0, -1)]
+    for a in bad:
+        assert L.sp_shell_create(*a[:3], a[3], a[4], a[5], C.byref(h)) == 1, a
+    assert L.sp_shell_create(9, 8, 16, 1.0, 3.0, 6, C.byref(h)) == 0
+    # hot calls before sp_build_matrices
+    assert L.sp_cartesian_gradient(h, 8, 1, 8, 8, 0, None) == 2
+    assert L.sp_get_matrix(h, 0, 0, 0, None, None, None) == 2
+    assert binding.status_string(2) == "SP_ERR_NOT_BUILT"
+    assert L.sp_shell_destroy(h) == 0
+
+
+@pytest.mark.parametrize("cfg", [(9, 8, 16, 1.0, 3.0, 6), (17, 24, 48, 1.8, 10.0, 19), (33, 48, 96, 1.8, 20.0, 43), (5, 7, 14, 1.0, 2.0, 4)])
+def test_host_matrices_match_oracle(cfg):
+    Nr, Nt, Np, rmin, rmax, L = cfg
+    sh = Shell(Nr, Nt, Np, rmin, rmax, L, host_only=True)
+    cd = sh.get_matrix(0)
+    ref = oracle.cheb_diff(Nr, rmin, rmax)
+    assert np.max(np.abs(cd - ref)) <= 4e-16 * np.max(np.abs(ref)) * 4
+    assert np.max(np.abs(sh.get_matrix(1) - oracle.fourier_diff(2 * Nt)[:Nt])) < 1e-14 * Nt
+    assert np.max(np.abs(sh.get_matrix(2) - oracle.fourier_diff(Np))) < 1e-14 * Nt
+    # Fourier rows (eq. 23-24 with B = sin, reading Q1): round trip synthesis(analysis) = identity on modes <= L
+    A, S = sh.get_matrix(3), sh.get_matrix(4)
+    assert A.shape == (2 * L + 1, Np) and S.shape == (Np, 2 * L + 1)
+    assert np.max(np.abs(A @ S - np.eye(2 * L + 1))) < 1e-14
+    ph = 2 * np.pi * np.arange(Np) / Np
+    for m in range(1, L + 1):
+        assert np.max(np.abs(S[:, 2 * m - 1] - np.cos(m * ph))) < 1e-13 and np.max(np.abs(S[:, 2 * m] - np.sin(m * ph))) < 1e-13
+    worst = 0.0
+    for n in range(-3, 4):
+        for m in range(0, L + 1):
+            worst = max(worst, np.max(np.abs(sh.get_matrix(5, n, m) - oracle.filter_matrix(Nt, L, n, m))))
+    assert worst < 1e-13, worst
