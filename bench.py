@@ -1,0 +1,406 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path (Cartesian gradient + Yn tensor filter, FP64) on B200.
+
+A "step" is one pass of the whole hot path over one synthetic state of the chosen configuration:
+sp_cartesian_gradient of all fields, then sp_tensor_filter of all tensors (SURVEY.md 8(a) rows G1-G4,
+F1-F5).  metric = grid-point*fields/s (BASELINE.json).  Contract: one JSON line on stdout (rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+N > 1 (torchrun): the path shards with no exchange step: every rank runs the full
+configuration on its own seeded state (independent shells), weak scaling, no data-path collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "grid-point*fields/s, gradient + Yn filter (FP64)"
+UNIT = "grid-point*fields/s"
+L2_BYTES = 126e6
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); default 3 = GHG-50 at 33x48x96")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def flops_per_unit(cfg):
+    """Algorithmic flops per grid-point*field: per stage."""
+    Nr, Nt, Np, L = cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["L"]
+    return {
+        "grad_dphi": 2.0 * Np,
+        "grad_rtheta": 2.0 * Nr + 4.0 * Nt + 13.0,
+        "filt_project": 0.0,
+        "filt_analysis": 2.0 * (2 * L + 1),
+        "filt_theta": 1.0 * (2 * L + 1),
+        "filt_synthesis": 2.0 * (2 * L + 1),
+        "filt_recombine": 0.0,
+    }
+
+
+def workload_name(cfg):
+    return (f"config {cfg['id']}: {cfg['nfields']} fields ({'+'.join(t['name'] for t in cfg['tensors'])}), "
+            f"Nr x Ntheta x Nphi = {cfg['Nr']}x{cfg['Nt']}x{cfg['Np']}, shell [{cfg['rmin']},{cfg['rmax']}], L = {cfg['L']}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.stop_flag, self.index = [], False, index
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def start(self):
+        self.t.start()
+
+    def stop(self):
+        self.stop_flag = True
+        self.t.join(timeout=6)
+        sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            for q, nm in enumerate(names):
+                if len(r) > 3 + q and r[3 + q].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None,
+                "sm_max_mhz": float(self.rows[0][1]) if self.rows and self.rows[0][1].replace(".", "").isdigit() else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference): the oracle as it stands, on a bounded sample
+# ---------------------------------------------------------------------------------------------------
+ORACLE_SAMPLE = {   # config -> (fields differentiated, radii filtered) of the FIRST tensor of the state
+    1: (1, 9), 2: (10, 17), 3: (4, 4), 4: (1, 1), 5: (1, 2),
+}
+
+
+def oracle_sample(cfg, u, threads):
+    """One bounded sample of the workload through the oracle.  Returns (seconds per unit, description).
+    A unit is one grid-point*field that went through the gradient AND the filter."""
+    import numpy as np
+    import oracle
+    oracle.set_threads(threads)
+    Nr, Nt, Np = cfg["Nr"], cfg["Nt"], cfg["Np"]
+    nfg, nrad = ORACLE_SAMPLE[cfg["id"]]
+    t0 = cfg["tensors"][0]
+    ug = np.ascontiguousarray(u[:nfg])
+    a = time.perf_counter()
+    oracle.gradient(ug, Nr, Nt, Np, cfg["rmin"], cfg["rmax"])
+    tg = time.perf_counter() - a
+    radii = [int(round(q * (Nr - 1) / max(nrad - 1, 1))) for q in range(nrad)] if nrad < Nr else list(range(Nr))
+    a = time.perf_counter()
+    if nrad >= Nr:
+        oracle.tensor_filter(u, Nr, Nt, Np, cfg["L"], [t0])
+    else:
+        for k in radii:
+            oracle.tensor_filter(u, Nr, Nt, Np, cfg["L"], [t0], ksel=k)
+    tf = time.perf_counter() - a
+    per_unit = tg / (nfg * Nr * Nt * Np) + tf / (len(t0["fields"]) * len(radii) * Nt * Np)
+    desc = (f"oracle (plain C, long double, OpenMP x{threads}): gradient of {nfg} field(s) on the full grid + Yn filter of "
+            f"tensor {t0['name']} at {len(radii)} of {Nr} radii (filter-matrix build included)")
+    return per_unit, tg + tf, desc
+
+
+def run_reference(args):
+    import numpy as np
+    import synth
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = synth.config(args.config)
+    u = synth.make_state(cfg)
+    threads = os.cpu_count() or 1
+    for _ in range(args.warmup):
+        oracle_sample(cfg, u, threads)
+    tot_units_time, wall, desc = 0.0, 0.0, ""
+    for _ in range(args.steps):
+        pu, w, desc = oracle_sample(cfg, u, threads)
+        tot_units_time += pu
+        wall += w
+    value = 1.0 / (tot_units_time / max(args.steps, 1))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# GPU leg
+# ---------------------------------------------------------------------------------------------------
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def aggregate_over_ranks(ms_local, units_local, dist=None):
+    """Whole-job numbers from per-rank ones: time = MAX over ranks, units = SUM over ranks.
+    (No data-path collective exists; these two scalars are the only cross-rank traffic.)"""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return ms_local, units_local
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([ms_local], dtype=torch.float64, device=dev)
+    n = torch.tensor([units_local], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(n.item())
+
+
+class GpuWorkload:
+    """State, outputs and workspaces of one configuration resident in HBM; step() = gradient + filter."""
+
+    def __init__(self, cfg, seed_offset=0, nsets=None):
+        import torch
+        import synth
+        from paper_1104_3408_b200 import Shell
+        self.torch, self.cfg = torch, cfg
+        self.sh = Shell(cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["rmin"], cfg["rmax"], cfg["L"])
+        u = synth.make_state(cfg, seed=cfg["seed"] + 1000 * seed_offset)
+        self.u_host = u
+        state_bytes = u.nbytes
+        # rotate over enough distinct input sets that consecutive steps never find their input in L2
+        self.nsets = nsets if nsets is not None else max(2, int(2 * L2_BYTES // state_bytes) + 1)
+        self.nsets = min(self.nsets, 8)
+        self.u = [torch.from_numpy(u).cuda() for _ in range(self.nsets)]
+        nf = cfg["nfields"]
+        self.du = torch.empty((3, nf, cfg["Np"], cfg["Nt"], cfg["Nr"]), dtype=torch.float64, device="cuda")
+        self.fu = torch.empty_like(self.u[0])
+        g, f, _ = self.sh.workspace_bytes(nf)
+        self.ws_g = torch.empty(g // 8, dtype=torch.float64, device="cuda")
+        self.ws_f = torch.empty(f // 8, dtype=torch.float64, device="cuda")
+        self.descs = self.sh.make_descs(cfg["tensors"])
+        self.units = float(cfg["npts"] * nf)
+        self.it = 0
+
+    def step(self):
+        u = self.u[self.it % self.nsets]
+        self.it += 1
+        self.sh.cartesian_gradient(u, out=self.du, workspace=self.ws_g)
+        self.sh.tensor_filter(u, self.cfg["tensors"], out=self.fu, workspace=self.ws_f, descs=self.descs)
+
+    def time_steps(self, steps, warmup):
+        torch = self.torch
+        for _ in range(warmup):
+            self.step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            self.step()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    def stage_times(self, reps=5):
+        """Per-stage device times (ms), median over reps, from CUDA events recorded inside the library
+        on the launching stream (sp_profile_enable)."""
+        import statistics
+        self.sh.profile(True)
+        rows = []
+        for _ in range(reps):
+            self.step()
+            rows.append(self.sh.profile_read())
+        self.sh.profile(False)
+        return {k: statistics.median(r[k] for r in rows) for k in rows[0]}
+
+    def e2e(self, steps):
+        """Same metric through the public API with HOST buffers: pinned host state -> device, gradient +
+        filter, results back to pinned host memory; copies inside the timed region."""
+        torch = self.torch
+        hu = torch.from_numpy(self.u_host).pin_memory()
+        hdu = torch.empty(self.du.shape, dtype=torch.float64).pin_memory()
+        hfu = torch.empty(self.fu.shape, dtype=torch.float64).pin_memory()
+        ud = self.u[0]
+
+        def one():
+            ud.copy_(hu, non_blocking=True)
+            self.sh.cartesian_gradient(ud, out=self.du, workspace=self.ws_g)
+            self.sh.tensor_filter(ud, self.cfg["tensors"], out=self.fu, workspace=self.ws_f, descs=self.descs)
+            hdu.copy_(self.du, non_blocking=True)
+            hfu.copy_(self.fu, non_blocking=True)
+
+        one()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            one()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        return ms, hu.numel() * 8, (hdu.numel() + hfu.numel()) * 8
+
+
+def roofline_for(cfg, stages_ms, units, peak_tf, hbm_gbs, hbm_src):
+    fl = flops_per_unit(cfg)
+    table = {}
+    for k, ms in stages_ms.items():
+        if ms is None or ms <= 0:
+            continue
+        table[k] = {"ms": ms, "tflops": fl[k] * units / (ms * 1e-3) * 1e-12}
+    dom = max(table, key=lambda k: table[k]["ms"])
+    ach = table[dom]["tflops"]
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(f"config{cfg['id']}", {}).get(dom)
+        except Exception:
+            traffic = None
+    roof = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
+            "traffic": traffic,
+            "peak_source": "FP64 DMMA issue peak measured live by sp_probe_fp64_peak (148 SMs x 64 FMA/clk x 2 x 1.965 GHz = 37.2 nominal)",
+            "hbm_gbs": hbm_gbs, "hbm_source": hbm_src}
+    return roof, table
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import synth
+    from paper_1104_3408_b200 import launch_count, probe_fp64_peak
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = synth.config(args.config)
+    wl = GpuWorkload(cfg, seed_offset=rank)
+    peak_tf = probe_fp64_peak(0)
+    hbm_gbs, hbm_src = measured_peaks()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    l0 = launch_count()
+    ms = wl.time_steps(args.steps, args.warmup)
+    launches = (launch_count() - l0) * args.steps // (args.steps + args.warmup)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    ms_all, units_all = aggregate_over_ranks(ms, wl.units * args.steps, dist if world > 1 else None)
+    value = units_all / (ms_all * 1e-3)
+
+    # end to end with host buffers (every rank, max over ranks)
+    e2e_ms, h2d, d2h = wl.e2e(max(3, min(args.steps, 10)))
+    e2e_ms_all, e2e_units = aggregate_over_ranks(e2e_ms, wl.units, dist if world > 1 else None)
+    stages = wl.stage_times()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+    roof, table = roofline_for(cfg, stages, wl.units, peak_tf, hbm_gbs, hbm_src)
+    fl = flops_per_unit(cfg)
+    tot_fl = sum(fl.values())
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "parallelism": f"replicas x{world} (independent shells, no collective)",
+                   "l2": f"inputs rotate over {wl.nsets} distinct state copies ({wl.nsets * wl.u_host.nbytes / 1e6:.0f} MB > 126 MB L2); "
+                         f"each step also streams {4 * wl.u_host.nbytes / 1e6:.0f} MB of outputs and the workspaces"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_units / (e2e_ms_all * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_ms_all},
+        "gpu_launches": int(launches),
+        "roofline": roof,
+        "path": {"algorithmic_flops_per_unit": tot_fl, "tflops": tot_fl * wl.units / (ms / args.steps * 1e-3) * 1e-12,
+                 "frac_of_fp64_peak": tot_fl * wl.units / (ms / args.steps * 1e-3) * 1e-12 / peak_tf,
+                 "hbm_min_bytes_per_unit": 48, "stages": table},
+        "fp64_peak_tflops": {"dmma": peak_tf, "dfma": probe_fp64_peak(1)},
+    }
+    if not args.no_others and world == 1:
+        others = {}
+        for cid in (2, 4, 5):
+            if cid == args.config:
+                continue
+            try:
+                del wl
+            except NameError:
+                pass
+            torch.cuda.empty_cache()
+            c2 = synth.config(cid)
+            w2 = GpuWorkload(c2)
+            k2 = 10 if cid != 2 else 50
+            m2 = w2.time_steps(k2, 3)
+            st2 = w2.stage_times()
+            r2, t2 = roofline_for(c2, st2, w2.units, peak_tf, hbm_gbs, hbm_src)
+            f2 = sum(flops_per_unit(c2).values())
+            others[f"config{cid}"] = {"workload": workload_name(c2), "value": w2.units * k2 / (m2 * 1e-3), "ms_per_step": m2 / k2,
+                                      "path_frac_of_fp64_peak": f2 * w2.units / (m2 / k2 * 1e-3) * 1e-12 / peak_tf,
+                                      "dominant": r2["kernel"], "dominant_frac": r2["frac"],
+                                      "stages_ms": {k: v["ms"] for k, v in t2.items()}}
+            wl = w2
+        line["other_configs"] = others
+    if not args.no_cpu_baseline and world == 1:
+        threads = os.cpu_count() or 1
+        pu, wall, desc = oracle_sample(cfg, synth.make_state(cfg), threads)
+        line["cpu_baseline"] = {"value": 1.0 / pu, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+                                "seconds": wall}
+    else:
+        line["cpu_baseline"] = None
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

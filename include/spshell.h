@@ -115,6 +115,16 @@ sp_status sp_get_matrix(const sp_shell *shell, int which, int n, int m, double *
  * loop; returns TFLOP/s.  Used by bench.py as the live denominator of the FP64 roofline. */
 sp_status sp_probe_fp64_peak(int mode, double *tflops_out);
 
+/* Per-stage device timing.  While enabled, the hot calls record CUDA events on the caller's stream
+ * between their stages; sp_profile_read synchronises on them and returns the last call's durations in
+ * milliseconds: ms7[0] d/dphi product, [1] d/dr + d/dtheta + chain rule, [2] dyad projection,
+ * [3] phi analysis, [4] theta matrices, [5] phi synthesis, [6] recombination (-1 if not recorded). */
+sp_status sp_profile_enable(sp_shell *shell, int on);
+sp_status sp_profile_read(const sp_shell *shell, double *ms7_host);
+
+/* Number of kernels the hot calls have launched since the library was loaded (host-side counter). */
+unsigned long long sp_launch_count(void);
+
 const char *sp_status_string(sp_status s);
 
 #ifdef __cplusplus

@@ -6,4 +6,4 @@ streams.  There is no CPU fallback: importing works anywhere (so the ABI can be 
 every compute call raises unless the CUDA library is built and a CUDA device is present.
 """
 from .binding import (SpError, Shell, lib, library_path, probe_fp64_peak, status_string,  # noqa: F401
-                      EXPORTED_SYMBOLS)
+                      EXPORTED_SYMBOLS, launch_count)

@@ -9,7 +9,7 @@ _lib = None
 EXPORTED_SYMBOLS = [
     "sp_shell_create", "sp_shell_destroy", "sp_build_matrices", "sp_workspace_bytes", "sp_cartesian_gradient",
     "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_axpby", "sp_get_matrix", "sp_probe_fp64_peak",
-    "sp_status_string",
+    "sp_status_string", "sp_profile_enable", "sp_profile_read", "sp_launch_count",
 ]
 
 
@@ -47,6 +47,10 @@ def lib():
         L.sp_axpby.argtypes = [C.c_double, C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_get_matrix.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.sp_probe_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
+        L.sp_profile_enable.argtypes = [C.c_void_p, C.c_int]
+        L.sp_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.sp_launch_count.restype = C.c_ulonglong
+        L.sp_launch_count.argtypes = []
         _lib = L
     return _lib
 
@@ -65,6 +69,10 @@ def probe_fp64_peak(mode=0):
     v = C.c_double()
     _check(lib().sp_probe_fp64_peak(mode, C.byref(v)), "sp_probe_fp64_peak")
     return v.value
+
+
+def launch_count():
+    return int(lib().sp_launch_count())
 
 
 def _stream_ptr(stream):
@@ -125,6 +133,17 @@ class Shell:
         out = np.zeros((r.value, c.value))
         _check(lib().sp_get_matrix(self._h, which, n, m, out.ctypes.data_as(C.c_void_p), C.byref(r), C.byref(c)), "sp_get_matrix")
         return out
+
+    STAGES = ("grad_dphi", "grad_rtheta", "filt_project", "filt_analysis", "filt_theta", "filt_synthesis", "filt_recombine")
+
+    def profile(self, on=True):
+        _check(lib().sp_profile_enable(self._h, 1 if on else 0), "sp_profile_enable")
+
+    def profile_read(self):
+        """dict stage -> milliseconds of the last profiled call(s)."""
+        ms = (C.c_double * 7)()
+        _check(lib().sp_profile_read(self._h, ms), "sp_profile_read")
+        return {k: ms[q] for q, k in enumerate(self.STAGES)}
 
     # ---- hot calls (marshalling only) ---------------------------------------------------------
     def cartesian_gradient(self, u, out=None, workspace=None, stream=None):

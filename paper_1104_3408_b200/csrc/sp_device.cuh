@@ -21,7 +21,18 @@ struct sp_shell {
     double *d_F = nullptr;         // F^n_m [7][L+1][Nt8][Nt4], zero padded            (eq. 62)
     double *d_inv_r = nullptr, *d_sin_t = nullptr, *d_cos_t = nullptr, *d_inv_sin_t = nullptr, *d_sin_p = nullptr,
            *d_cos_p = nullptr;     // Jacobian / triad factors                          (eq. 6, 51)
+    // optional per-stage timing (sp_profile_enable): events recorded on the caller's stream
+    mutable bool prof = false;
+    mutable cudaEvent_t ev[9] = {};
+    mutable bool ev_set[9] = {};
 };
+
+// stage marks: 0 grad start, 1 after d/dphi, 2 after r-theta+chain rule, 3 filter start, 4 after projection,
+// 5 after phi analysis, 6 after theta matrices, 7 after phi synthesis, 8 after recombination
+static inline void sp_mark(const sp_shell *s, cudaStream_t st, int idx) {
+    if (s->prof) { cudaEventRecord(s->ev[idx], st); s->ev_set[idx] = true; }
+}
+extern unsigned long long g_sp_launches;   // kernels launched by hot calls since load (host counter)
 
 sp_status sp_configure_kernels(sp_shell *s);
 

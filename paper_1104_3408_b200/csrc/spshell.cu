@@ -16,6 +16,8 @@
         if (e_ != cudaSuccess) return SP_ERR_CUDA;   \
     } while (0)
 
+unsigned long long g_sp_launches = 0;
+
 static int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
 extern "C" const char *sp_status_string(sp_status s) {
@@ -62,6 +64,8 @@ static void free_dev(sp_shell *s) {
 extern "C" sp_status sp_shell_destroy(sp_shell *s) {
     if (!s) return SP_ERR_INVALID_ARG;
     free_dev(s);
+    for (int q = 0; q < 9; q++)
+        if (s->ev[q]) cudaEventDestroy(s->ev[q]);
     delete s->host;
     delete s;
     return SP_OK;
@@ -192,18 +196,22 @@ extern "C" sp_status sp_workspace_bytes(const sp_shell *s, int nfields, size_t *
 
 extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, int nf, double *du, void *ws, size_t wsb,
                                            void *stream) {
-    if (!s || !u || !du || nf < 0) return SP_ERR_INVALID_ARG;
+    if (!s || nf < 0) return SP_ERR_INVALID_ARG;
     if (!s->built) return SP_ERR_NOT_BUILT;
-    if (nf == 0) return SP_OK;
+    if (nf == 0) return SP_OK;                          // empty input: nothing to do (pointers may be null)
+    if (!u || !du) return SP_ERR_INVALID_ARG;
     if (!ws || wsb < (size_t)nf * s->npts * sizeof(double)) return SP_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const int Nr = s->Nr, Nt = s->Nt, Np = s->Np;
     const long plane = (long)Nr * Nt;
     double *dphi = (double *)ws;
+    sp_mark(s, st, 0);
     // d/dphi: FD_{Np} (circulant) over j, stride Nr*Nt; every field is one batch          (eq. 8, 18)
     sp_status e = launch_gemm_cols<true>(s->d_g3, Np, Np, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts,
                                          (int)plane, nf, st);
     if (e != SP_OK) return e;
+    sp_mark(s, st, 1);
+    g_sp_launches += 2;
     GradParams p;
     p.Nr = Nr; p.Nt = Nt; p.Np = Np; p.PU = s->PU; p.Nr8 = s->Nr8; p.Nr4 = s->Nr4; p.Nt8 = s->Nt8;
     p.cd = s->d_cd; p.g2 = s->d_g2;
@@ -222,6 +230,7 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         int nw = ntasks < 16 ? ntasks : 16;
         k_grad_rtheta<5><<<grid, nw * 32, sm, st>>>(p);
     }
+    sp_mark(s, st, 2);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
 
@@ -336,11 +345,15 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     if (!ws || wsb < need) return SP_ERR_INVALID_ARG;
     double *dofs = (double *)ws, *coef1 = dofs + (size_t)ndof * npts, *coef2 = coef1 + (size_t)ndof * s->MC4 * vec;
     // ---- F1: dyad projection
+    sp_mark(s, st, 3);
     for (int t = 0; t < ntens; t++) launch_pointwise<false>(types[t], targs[t], s, u, dofs, st);
+    sp_mark(s, st, 4);
+    g_sp_launches += 2 * ntens + 2 + (comps.size() + SP_THETA_BATCH - 1) / SP_THETA_BATCH;
     // ---- F2: phi analysis (eq. 33)
     sp_status e = launch_gemm_cols<false>(s->d_an, Np, s->MC, Np, dofs, (long)vec, (long)npts, coef1, (long)vec,
                                           (long)(s->MC4 * vec), (int)vec, ndof, st);
     if (e != SP_OK) return e;
+    sp_mark(s, st, 5);
     // ---- F3: per-(n,m) theta matrices (eq. 62)
     {
         const int nwarps = (Nr + 3) / 4, mtiles = s->Nt8 / 8;
@@ -359,12 +372,15 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
         }
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
     }
+    sp_mark(s, st, 6);
     // ---- F4: phi synthesis (eq. 31)
     e = launch_gemm_cols<false>(s->d_sy, s->MC4, Np, s->MC, coef2, (long)vec, (long)(s->MC4 * vec), dofs, (long)vec, (long)npts,
                                 (int)vec, ndof, st);
     if (e != SP_OK) return e;
+    sp_mark(s, st, 7);
     // ---- F5: recombination
     for (int t = 0; t < ntens; t++) launch_pointwise<true>(types[t], targs[t], s, dofs, out, st);
+    sp_mark(s, st, 8);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
 
@@ -377,6 +393,7 @@ extern "C" sp_status sp_rhs_first_order_wave(const sp_shell *s, const double *u,
     sp_status e = sp_cartesian_gradient(s, u + npts, 4, dg, gws, 4 * npts * sizeof(double), stream);
     if (e != SP_OK) return e;
     const int T = 256;
+    g_sp_launches += 1;
     k_wave_rhs<<<(unsigned)((npts + T - 1) / T), T, 0, (cudaStream_t)stream>>>(s->Nr, s->Nt, npts, s->d_sin_t, s->d_cos_t, s->d_sin_p,
                                                                               s->d_cos_p, u, dg, dudt);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
@@ -387,6 +404,7 @@ extern "C" sp_status sp_axpby(double a, const double *x, double b, double *y, si
     if (n == 0) return SP_OK;
     size_t nb = (n + 255) / 256;
     if (nb > 148 * 16) nb = 148 * 16;
+    g_sp_launches += 1;
     k_axpby<<<(unsigned)nb, 256, 0, (cudaStream_t)stream>>>(a, x, b, y, n);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
@@ -417,3 +435,30 @@ extern "C" sp_status sp_probe_fp64_peak(int mode, double *tflops) {
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(buf);
     return SP_OK;
 }
+
+extern "C" sp_status sp_profile_enable(sp_shell *s, int on) {
+    if (!s) return SP_ERR_INVALID_ARG;
+    if (on)
+        for (int q = 0; q < 9; q++)
+            if (!s->ev[q]) SP_CUDA(cudaEventCreate(&s->ev[q]));
+    for (int q = 0; q < 9; q++) s->ev_set[q] = false;
+    s->prof = on != 0;
+    return SP_OK;
+}
+
+extern "C" sp_status sp_profile_read(const sp_shell *s, double *ms7) {
+    if (!s || !ms7) return SP_ERR_INVALID_ARG;
+    static const int a[7] = {0, 1, 3, 4, 5, 6, 7}, b[7] = {1, 2, 4, 5, 6, 7, 8};
+    for (int q = 0; q < 7; q++) {
+        ms7[q] = -1.0;
+        if (s->ev_set[a[q]] && s->ev_set[b[q]]) {
+            SP_CUDA(cudaEventSynchronize(s->ev[b[q]]));
+            float ms = 0;
+            SP_CUDA(cudaEventElapsedTime(&ms, s->ev[a[q]], s->ev[b[q]]));
+            ms7[q] = ms;
+        }
+    }
+    return SP_OK;
+}
+
+extern "C" unsigned long long sp_launch_count(void) { return g_sp_launches; }
