@@ -178,3 +178,35 @@ def tensor_filter(u, Nr, Nt, Np, L, tensors, ksel=-1):
                             C.c_int(nt), rank.ctypes, dims.ctypes, sym.ctypes, foff.ctypes, fields.ctypes,
                             C.c_int(ksel))
     return out
+
+
+def wave_rhs(u, Nr, Nt, Np, rmin, rmax):
+    """RHS of the first-order scalar wave system with the freezing boundary condition (O13)."""
+    u, nf = _state(u, Nr, Nt, Np)
+    assert nf == 5
+    out = np.empty_like(u)
+    lib().orc_wave_rhs(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_double(rmin), C.c_double(rmax), u.ctypes, out.ctypes)
+    return out
+
+
+def wave_dt(Nr, Nt, Np, rmin, rmax, lam=4.0):
+    """dt = lambda * min(dx) (eq. 63; reading W4): min over the radial spacing at the
+    inner boundary and the azimuthal spacing on the innermost shell next to the pole."""
+    r, th, ph = grid(Nr, Nt, Np, rmin, rmax)
+    dphi = 2.0 * r[0] * np.sin(th[0]) * np.sin(np.pi / Np)
+    return lam * min(r[1] - r[0], dphi)
+
+
+def wave_rk4(u, Nr, Nt, Np, rmin, rmax, L, tensors, dt, nsteps):
+    """Classical RK4 with the Yn filter applied to the initial data, to every stage
+    state before its RHS and to the final combination: 4 filters per step (reading W5)."""
+    F = lambda v: tensor_filter(v, Nr, Nt, Np, L, tensors)
+    R = lambda v: wave_rhs(v, Nr, Nt, Np, rmin, rmax)
+    u = F(np.array(u, dtype=np.float64))
+    for _ in range(nsteps):
+        k1 = R(u)
+        k2 = R(F(u + 0.5 * dt * k1))
+        k3 = R(F(u + 0.5 * dt * k2))
+        k4 = R(F(u + dt * k3))
+        u = F(u + dt / 6.0 * (k1 + 2.0 * k2 + 2.0 * k3 + k4))
+    return u

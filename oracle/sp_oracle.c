@@ -400,9 +400,16 @@ void orc_spin_analysis(int N, int n, int m, const double *s, double *cout) {
  * built directly from eq. (48) with that (n, m) -- no symmetry is assumed (reading Q12).
  * tab[((n+nmax)*(2N-1) + (m+N-1))*N*N + i*N + ii], double.
  * ---------------------------------------------------------------------------------- */
+/* The last table is kept (it depends on (N, L, nmax) only and the time loop of O13 asks for the same
+ * one thousands of times); callers must not free it. */
 static double *filter_table(int N, int L, int nmax) {
+    static int cN = -1, cL = -1, cn = -1;
+    static double *ctab = NULL;
+    if (ctab && cN == N && cL == L && cn == nmax) return ctab;
+    free(ctab);
+    cN = N; cL = L; cn = nmax;
     int nm = 2 * N - 1, nn = 2 * nmax + 1;
-    double *tab = malloc(sizeof(double) * (size_t)nn * nm * N * N);
+    double *tab = ctab = malloc(sizeof(double) * (size_t)nn * nm * N * N);
 #pragma omp parallel for collapse(2) schedule(dynamic)
     for (int n = -nmax; n <= nmax; n++)
         for (int m = -(N - 1); m <= N - 1; m++)
@@ -630,5 +637,47 @@ void orc_tensor_filter(int Nr, int Nt, int Np, int L, int nfields, const double 
             tensor_filter_sphere(Nr, Nt, Np, Ftab, nmax, k, rank[t], dims + 3 * t, sym[2 * t], sym[2 * t + 1],
                                  fields + foff[t], u, res);
     if (out == u) { memcpy(out, res, sizeof(double) * tot); free(res); }
-    free(Ftab);
+}
+
+/* ------------------------------------------------------------------------------------
+ * O13  First-order scalar wave system on the shell (BASELINE.json config 5).  The paper
+ * has no scalar-wave system of its own; this is its class of problems, eq. (1)
+ * (PAPER.md:19), specialised from the GHG first-order reduction (A.6-A.8)
+ * and its characteristic machinery (A.13-A.16) to flat space
+ * (readings W1-W3):
+ *   u = (psi, Pi, Phi_x, Phi_y, Phi_z),  Pi = -d_t psi,  Phi_i = d_i psi
+ *   d_t psi = -Pi;   d_t Pi = -(d_x Phi_x + d_y Phi_y + d_z Phi_z);   d_t Phi_i = -d_i Pi
+ * Boundary shells k = 0 (outward normal s = -r^) and k = Nr-1 (s = +r^): characteristic fields
+ * U^+- = Pi +- s.Phi (speeds +-1), zero-speed psi and tangential Phi.  Freeze the incoming
+ * field (A.16): with d the computed RHS,  U = d_Pi + s.d_Phi;  d_Pi <- U/2;
+ * d_Phi_i <- d_Phi_i - s_i (s.d_Phi) + s_i U/2;  d_psi unchanged.
+ * ---------------------------------------------------------------------------------- */
+void orc_wave_rhs(int Nr, int Nt, int Np, double rmin, double rmax, const double *u, double *dudt) {
+    size_t npts = (size_t)Nr * Nt * Np;
+    double *dg = malloc(sizeof(double) * 12 * npts);          /* [3][4]: gradient of Pi, Phi_x, Phi_y, Phi_z */
+    orc_gradient(Nr, Nt, Np, 4, rmin, rmax, u + npts, dg);
+    for (int j = 0; j < Np; j++)
+        for (int i = 0; i < Nt; i++)
+            for (int k = 0; k < Nr; k++) {
+                size_t p = (size_t)k + (size_t)Nr * (i + (size_t)Nt * j);
+#define DG(c, f) dg[((size_t)(c) * 4 + (f)) * npts + p]
+                ld dpsi = -(ld)u[npts + p];
+                ld dPi = -((ld)DG(0, 1) + (ld)DG(1, 2) + (ld)DG(2, 3));
+                ld dPh[3] = { -(ld)DG(0, 0), -(ld)DG(1, 0), -(ld)DG(2, 0) };
+#undef DG
+                if (k == 0 || k == Nr - 1) {
+                    ld th = grid_th(Nt, i), ph = grid_ph(Np, j), sg = (k == 0) ? -1 : 1;
+                    ld s[3] = { sg * sinl(th) * cosl(ph), sg * sinl(th) * sinl(ph), sg * cosl(th) };
+                    ld sd = s[0] * dPh[0] + s[1] * dPh[1] + s[2] * dPh[2];
+                    ld U = dPi + sd;
+                    dPi = U / 2;
+                    for (int c = 0; c < 3; c++) dPh[c] = dPh[c] - s[c] * sd + s[c] * U / 2;
+                }
+                dudt[p] = (double)dpsi;
+                dudt[npts + p] = (double)dPi;
+                dudt[2 * npts + p] = (double)dPh[0];
+                dudt[3 * npts + p] = (double)dPh[1];
+                dudt[4 * npts + p] = (double)dPh[2];
+            }
+    free(dg);
 }
