@@ -1,0 +1,136 @@
+// phi-direction contraction, shared-memory staged (the hot GEMM: d/dphi, phi analysis, phi synthesis).
+//     C[b][m][c] = sum_k A[m][k] * B[b][k][c],   B[b][k][c] = B + b*sBb + k*sBk + c  (columns contiguous)
+// (eq. 17-19 without the transposes; 254-259 eq. 33; 243-246 eq. 31.)
+// CTA tile = ALL rows of A x 64 columns; K walked in chunks of 8 through a 4-stage cp.async pipeline:
+//   As[stage][Mpad][12]  (pitch 12 doubles: fragment reads hit 16 distinct 8-byte banks)
+//   Bs[stage][8][68]     (pitch 68 = 4 mod 16: likewise)
+// Warp (mg, ng): MT m-tiles x 2 n-tiles of 8x8, DMMA.8x8x4.  Requires even strides / ncols and 16-byte
+// aligned bases (checked by the launcher; otherwise the generic kernel of kernels_gemm.cuh is used).
+#pragma once
+#include "sp_device.cuh"
+
+#include <cstdint>
+
+#define PG_NCOL 64
+#define PG_KC 8
+#define PG_STAGES 4
+#define PG_PA 12
+#define PG_PB 68
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+template <int MT>
+__global__ void __launch_bounds__(512)
+k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const double *__restrict__ B, long sBk, long sBb,
+           double *__restrict__ C, long sCm, long sCb, int ncols) {
+    extern __shared__ __align__(16) double sm[];
+    const int stageA = Mpad * PG_PA, stageB = PG_KC * PG_PB;
+    double *As = sm, *Bs = sm + PG_STAGES * stageA;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    const int mg = warp >> 2, ng = warp & 3;
+    const int c0 = blockIdx.x * PG_NCOL;
+    const double *Bb = B + (long)blockIdx.y * sBb + c0;
+    double *Cb = C + (long)blockIdx.y * sCb + c0;
+    const int nchunks = (K + PG_KC - 1) / PG_KC;
+    const int colsleft = ncols - c0;                    // > 0, even
+
+    auto load_chunk = [&](int kc, int st) {
+        // A chunk: Mpad rows x 8 doubles (4 x 16 B per row); rows and K are zero padded in global memory
+        double *as = As + st * stageA;
+        for (int q = tid; q < Mpad * 4; q += blockDim.x) {
+            const int r = q >> 2, h = q & 3;
+            cp_async16(as + r * PG_PA + 2 * h, A + (long)r * lda + kc * PG_KC + 2 * h);
+        }
+        // B chunk: 8 rows x 64 columns (32 x 16 B per row); rows >= K and columns >= ncols are zero-filled
+        double *bs = Bs + st * stageB;
+        for (int q = tid; q < PG_KC * (PG_NCOL / 2); q += blockDim.x) {
+            const int r = q >> 5, h = q & 31;
+            const int k = kc * PG_KC + r;
+            double *dst = bs + r * PG_PB + 2 * h;
+            if (k < K && 2 * h < colsleft) cp_async16(dst, Bb + (long)k * sBk + 2 * h);
+            else { dst[0] = 0.0; dst[1] = 0.0; }
+        }
+    };
+
+    double acc[MT][2][2];
+#pragma unroll
+    for (int a = 0; a < MT; a++)
+#pragma unroll
+        for (int b = 0; b < 2; b++) acc[a][b][0] = acc[a][b][1] = 0.0;
+
+#pragma unroll
+    for (int s = 0; s < PG_STAGES - 1; s++) {
+        if (s < nchunks) load_chunk(s, s);
+        cp_async_commit();
+    }
+    for (int kc = 0; kc < nchunks; kc++) {
+        cp_async_wait<PG_STAGES - 2>();
+        __syncthreads();
+        if (kc + PG_STAGES - 1 < nchunks) load_chunk(kc + PG_STAGES - 1, (kc + PG_STAGES - 1) % PG_STAGES);
+        cp_async_commit();
+        const double *as = As + (kc % PG_STAGES) * stageA + (mg * MT * 8 + g) * PG_PA + t;
+        const double *bs = Bs + (kc % PG_STAGES) * stageB + t * PG_PB + ng * 16 + g;
+#pragma unroll
+        for (int ks = 0; ks < PG_KC / 4; ks++) {
+            double af[MT], bf[2];
+#pragma unroll
+            for (int a = 0; a < MT; a++) af[a] = as[a * 8 * PG_PA + ks * 4];
+            bf[0] = bs[ks * 4 * PG_PB];
+            bf[1] = bs[ks * 4 * PG_PB + 8];
+#pragma unroll
+            for (int a = 0; a < MT; a++) {
+                dmma(acc[a][0][0], acc[a][0][1], af[a], bf[0]);
+                dmma(acc[a][1][0], acc[a][1][1], af[a], bf[1]);
+            }
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < MT; a++) {
+        const int row = (mg * MT + a) * 8 + g;
+        if (row >= M) continue;
+#pragma unroll
+        for (int b = 0; b < 2; b++) {
+            const int col = ng * 16 + b * 8 + 2 * t;
+            if (col < colsleft) *reinterpret_cast<double2 *>(Cb + (long)row * sCm + col) = make_double2(acc[a][b][0], acc[a][b][1]);
+        }
+    }
+}
+
+// tiling of the row dimension chosen at build time: MT in {4,5,6} m-tiles per warp, mgroups warps along M
+struct PhiTiling { int MT, mgroups, Mpad; };
+static inline PhiTiling phi_tiling(int M) {
+    const int mtiles = (M + 7) / 8;
+    PhiTiling best = {6, (mtiles + 5) / 6, 0};
+    int bestpad = best.mgroups * 6;
+    for (int mt = 5; mt >= 4; mt--) {
+        int gq = (mtiles + mt - 1) / mt;
+        if (gq * mt < bestpad && gq <= 4) { best.MT = mt; best.mgroups = gq; bestpad = gq * mt; }
+    }
+    if (best.mgroups > 4) { best.MT = 6; best.mgroups = (mtiles + 5) / 6; }
+    best.Mpad = best.mgroups * best.MT * 8;
+    return best;
+}
+static inline size_t phi_smem_bytes(const PhiTiling &tl) {
+    return (size_t)PG_STAGES * ((size_t)tl.Mpad * PG_PA + PG_KC * PG_PB) * sizeof(double);
+}
+
+// returns SP_ERR_UNSUPPORTED when the fast-path preconditions do not hold (caller falls back)
+static sp_status launch_phi_gemm(const double *A, int lda, int M, const PhiTiling &tl, int K, const double *B, long sBk, long sBb,
+                                 double *C, long sCm, long sCb, int ncols, int nbatch, cudaStream_t st) {
+    if ((sBk | sBb | sCm | sCb | (long)ncols) & 1) return SP_ERR_UNSUPPORTED;
+    if (((uintptr_t)B | (uintptr_t)C) & 15) return SP_ERR_UNSUPPORTED;
+    if (tl.mgroups > 4) return SP_ERR_UNSUPPORTED;
+    dim3 grid((ncols + PG_NCOL - 1) / PG_NCOL, nbatch), block(tl.mgroups * 4 * 32);
+    const size_t sm = phi_smem_bytes(tl);
+    switch (tl.MT) {
+        case 4: k_phi_gemm<4><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols); break;
+        case 5: k_phi_gemm<5><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols); break;
+        default: k_phi_gemm<6><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols); break;
+    }
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}

@@ -3,8 +3,10 @@
 #include "../../include/spshell.h"
 #include "sp_internal.h"
 #include "sp_device.cuh"
+#include "kernels_gemm2.cuh"
 
 #include <cuda_runtime.h>
+#include <cstdint>
 
 #include <cstdio>
 #include <cstring>
@@ -53,7 +55,7 @@ extern "C" sp_status sp_shell_create(int Nr, int Nt, int Np, double rin, double 
 }
 
 static void free_dev(sp_shell *s) {
-    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
+    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_fd3p, &s->d_anp, &s->d_syp, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
                     &s->d_inv_sin_t, &s->d_sin_p, &s->d_cos_p};
     for (auto q : p) {
         if (*q) cudaFree(*q);
@@ -116,6 +118,23 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
                 for (int j = 0; j < Nt; j++)
                     f[((size_t)q * s->Nt8 + i) * s->Nt4 + j] = H.F[((size_t)q * Nt + i) * Nt + j];
         if ((st = upload(&s->d_F, f.data(), f.size())) != SP_OK) return st;
+    }
+    {   // padded operands of k_phi_gemm
+        PhiTiling t1 = phi_tiling(Np), t2 = phi_tiling(s->MC), t3 = phi_tiling(Np);
+        s->fd3_MT = t1.MT; s->fd3_mg = t1.mgroups; s->fd3_Mpad = t1.Mpad;
+        s->an_MT = t2.MT; s->an_mg = t2.mgroups; s->an_Mpad = t2.Mpad;
+        s->sy_MT = t3.MT; s->sy_mg = t3.mgroups; s->sy_Mpad = t3.Mpad;
+        s->Np8 = round_up(Np, 8); s->MCk8 = round_up(s->MC, 8);
+        std::vector<double> a((size_t)t1.Mpad * s->Np8, 0.0), b((size_t)t2.Mpad * s->Np8, 0.0), c((size_t)t3.Mpad * s->MCk8, 0.0);
+        for (int i = 0; i < Np; i++)
+            for (int j = 0; j < Np; j++) a[(size_t)i * s->Np8 + j] = H.g3[((i - j) % Np + Np) % Np];
+        for (int m = 0; m < s->MC; m++)
+            for (int j = 0; j < Np; j++) b[(size_t)m * s->Np8 + j] = H.an[(size_t)m * Np + j];
+        for (int j = 0; j < Np; j++)
+            for (int m = 0; m < s->MC; m++) c[(size_t)j * s->MCk8 + m] = H.sy[(size_t)j * s->MC + m];
+        if ((st = upload(&s->d_fd3p, a.data(), a.size())) != SP_OK) return st;
+        if ((st = upload(&s->d_anp, b.data(), b.size())) != SP_OK) return st;
+        if ((st = upload(&s->d_syp, c.data(), c.size())) != SP_OK) return st;
     }
     if ((st = upload(&s->d_inv_r, H.inv_r.data(), Nr)) != SP_OK) return st;
     if ((st = upload(&s->d_sin_t, H.sin_t.data(), Nt)) != SP_OK) return st;
@@ -182,6 +201,10 @@ sp_status sp_configure_kernels(sp_shell *s) {
     if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;       // (r,theta) plane pair must fit one SM's shared memory
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const int pg = (int)((size_t)PG_STAGES * ((size_t)4 * 6 * 8 * PG_PA + PG_KC * PG_PB) * sizeof(double));
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     return SP_OK;
 }
 
@@ -207,8 +230,10 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     double *dphi = (double *)ws;
     sp_mark(s, st, 0);
     // d/dphi: FD_{Np} (circulant) over j, stride Nr*Nt; every field is one batch          (eq. 8, 18)
-    sp_status e = launch_gemm_cols<true>(s->d_g3, Np, Np, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts,
-                                         (int)plane, nf, st);
+    PhiTiling tl = {s->fd3_MT, s->fd3_mg, s->fd3_Mpad};
+    sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
+    if (e == SP_ERR_UNSUPPORTED)   // odd strides: generic global-memory kernel
+        e = launch_gemm_cols<true>(s->d_g3, Np, Np, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
     if (e != SP_OK) return e;
     sp_mark(s, st, 1);
     g_sp_launches += 2;
@@ -350,8 +375,12 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     sp_mark(s, st, 4);
     g_sp_launches += 2 * ntens + 2 + (comps.size() + SP_THETA_BATCH - 1) / SP_THETA_BATCH;
     // ---- F2: phi analysis (eq. 33)
-    sp_status e = launch_gemm_cols<false>(s->d_an, Np, s->MC, Np, dofs, (long)vec, (long)npts, coef1, (long)vec,
-                                          (long)(s->MC4 * vec), (int)vec, ndof, st);
+    PhiTiling tla = {s->an_MT, s->an_mg, s->an_Mpad}, tls = {s->sy_MT, s->sy_mg, s->sy_Mpad};
+    sp_status e = launch_phi_gemm(s->d_anp, s->Np8, s->MC, tla, Np, dofs, (long)vec, (long)npts, coef1, (long)vec, (long)(s->MC4 * vec),
+                                  (int)vec, ndof, st);
+    if (e == SP_ERR_UNSUPPORTED)
+        e = launch_gemm_cols<false>(s->d_an, Np, s->MC, Np, dofs, (long)vec, (long)npts, coef1, (long)vec, (long)(s->MC4 * vec),
+                                    (int)vec, ndof, st);
     if (e != SP_OK) return e;
     sp_mark(s, st, 5);
     // ---- F3: per-(n,m) theta matrices (eq. 62)
@@ -374,8 +403,11 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     }
     sp_mark(s, st, 6);
     // ---- F4: phi synthesis (eq. 31)
-    e = launch_gemm_cols<false>(s->d_sy, s->MC4, Np, s->MC, coef2, (long)vec, (long)(s->MC4 * vec), dofs, (long)vec, (long)npts,
-                                (int)vec, ndof, st);
+    e = launch_phi_gemm(s->d_syp, s->MCk8, Np, tls, s->MC, coef2, (long)vec, (long)(s->MC4 * vec), dofs, (long)vec, (long)npts, (int)vec,
+                        ndof, st);
+    if (e == SP_ERR_UNSUPPORTED)
+        e = launch_gemm_cols<false>(s->d_sy, s->MC4, Np, s->MC, coef2, (long)vec, (long)(s->MC4 * vec), dofs, (long)vec, (long)npts,
+                                    (int)vec, ndof, st);
     if (e != SP_OK) return e;
     sp_mark(s, st, 7);
     // ---- F5: recombination
