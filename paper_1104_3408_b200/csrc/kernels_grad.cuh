@@ -109,3 +109,122 @@ __global__ void __launch_bounds__(512) k_grad_rtheta(GradParams p) {
         }
     }
 }
+
+// ---------------------------------------------------------------------------------------------
+// v2 of the (r,theta)-plane kernel: same mathematics and data flow as k_grad_rtheta, but
+//   * warp task = (plane, PAIR of latitude tiles, group of 3 radial tiles): every A fragment feeds 3 and
+//     every B fragment 2 DMMAs (0.83 shared-memory loads per DMMA instead of 1.2);
+//   * <= 85 registers so that two CTAs share an SM and one CTA's plane load / epilogue overlaps the
+//     other's tensor work; planes arrive by 8-byte cp.async while the CD^ table is copied;
+//   * only the padding (columns >= Nr, rows >= Nt) is zero-filled.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cp_async8g(void *smem, const void *gmem) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gmem));
+}
+
+#define GR_KT 3
+__global__ void __launch_bounds__(384, 2) k_grad_rtheta2(GradParams p) {
+    extern __shared__ double sm[];
+    const int Nr = p.Nr, Nt = p.Nt, Np = p.Np, PU = p.PU;
+    double *P0 = sm, *P1 = sm + (size_t)p.Nt8 * PU, *CDs = P1 + (size_t)p.Nt8 * PU, *g2s = CDs + (size_t)p.Nr8 * PU;
+    const int j = blockIdx.x, mu = blockIdx.y;
+    const size_t npts = (size_t)Nr * Nt * Np, plane = (size_t)Nr * Nt;
+    const double *u0 = p.u + mu * npts + (size_t)j * plane, *u1 = u0 + (size_t)Nt * plane;
+
+    // planes: asynchronous 8-byte copies into the padded pitch
+    for (int q = threadIdx.x; q < Nt * Nr; q += blockDim.x) {
+        const int i = q / Nr, k = q - i * Nr;
+        cp_async8g(P0 + i * PU + k, u0 + q);
+        cp_async8g(P1 + i * PU + k, u1 + q);
+    }
+    asm volatile("cp.async.commit_group;\n" ::);
+    // padding of the planes
+    const int padc = PU - Nr;
+    for (int q = threadIdx.x; q < Nt * padc; q += blockDim.x) {
+        const int i = q / padc, k = Nr + (q - i * padc);
+        P0[i * PU + k] = 0.0; P1[i * PU + k] = 0.0;
+    }
+    for (int q = threadIdx.x; q < (p.Nt8 - Nt) * PU; q += blockDim.x) { P0[Nt * PU + q] = 0.0; P1[Nt * PU + q] = 0.0; }
+    for (int q = threadIdx.x; q < p.Nr8 * PU; q += blockDim.x) CDs[q] = __ldg(p.cd + q);
+    for (int q = threadIdx.x; q < 2 * Nt; q += blockDim.x) g2s[q] = __ldg(p.g2 + q);
+    asm volatile("cp.async.wait_group 0;\n" ::);
+    __syncthreads();
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int itiles = p.Nt8 >> 3, ipairs = (itiles + 1) >> 1, ktiles = p.Nr8 >> 3, kgroups = (ktiles + GR_KT - 1) / GR_KT;
+    const int ntasks = 2 * ipairs * kgroups;
+    const int n2 = 2 * Nt;
+    for (int task = warp; task < ntasks; task += nwarps) {
+        const int pl = task / (ipairs * kgroups);
+        const int rem = task - pl * ipairs * kgroups;
+        const int ip = rem / kgroups, kg = rem - ip * kgroups;
+        const double *Pown = pl ? P1 : P0, *Poth = pl ? P0 : P1;
+        const int kt0 = kg * GR_KT;
+        const int ir0 = ip * 16 + g, ir1 = ir0 + 8;          // the lane's two latitude rows
+        const bool r1ok = (ip * 2 + 1) < itiles;
+        double at[2][GR_KT][2], ar[2][GR_KT][2];
+#pragma unroll
+        for (int a = 0; a < 2; a++)
+#pragma unroll
+            for (int q = 0; q < GR_KT; q++) at[a][q][0] = at[a][q][1] = ar[a][q][0] = ar[a][q][1] = 0.0;
+        // ---- d/dtheta over the extended latitude index ii = 4 ks + t (eq. 8 with the double cover)
+        int d0 = ir0 - t; d0 += (d0 < 0) ? n2 : 0;
+        int d1 = ir1 - t; d1 += (d1 < 0) ? n2 : 0; d1 -= (d1 >= n2) ? n2 : 0;
+        const int ksteps = (n2 + 3) >> 2;
+        for (int ks = 0; ks < ksteps; ks++) {
+            const int ii = ks * 4 + t;
+            const bool iok = ii < n2;
+            const double a0 = (iok && ir0 < Nt) ? g2s[d0] : 0.0;
+            const double a1 = (iok && r1ok && ir1 < Nt) ? g2s[d1] : 0.0;
+            d0 -= 4; d0 += (d0 < 0) ? n2 : 0;
+            d1 -= 4; d1 += (d1 < 0) ? n2 : 0;
+            const int iic = iok ? ii : n2 - 1;
+            const double *rowp = ((iic < Nt) ? (Pown + iic * PU) : (Poth + (n2 - 1 - iic) * PU)) + kt0 * 8 + g;
+#pragma unroll
+            for (int q = 0; q < GR_KT; q++) {
+                const double bf = (kt0 + q < ktiles) ? rowp[q * 8] : 0.0;
+                dmma(at[0][q][0], at[0][q][1], a0, bf);
+                dmma(at[1][q][0], at[1][q][1], a1, bf);
+            }
+        }
+        // ---- d/dr: A = u[i][kk], B[kk][k'] = CD^[k'][kk]   (eq. 9, 13)
+        const double *arow0 = Pown + ir0 * PU + t, *arow1 = Pown + (r1ok ? ir1 : ir0) * PU + t;
+        const double *cdp = CDs + (kt0 * 8 + g) * PU + t;
+        for (int ks = 0; ks < p.Nr4 / 4; ks++) {
+            const double a0 = arow0[ks * 4], a1 = arow1[ks * 4];
+#pragma unroll
+            for (int q = 0; q < GR_KT; q++) {
+                const double bf = (kt0 + q < ktiles) ? cdp[q * 8 * PU + ks * 4] : 0.0;
+                dmma(ar[0][q][0], ar[0][q][1], a0, bf);
+                dmma(ar[1][q][0], ar[1][q][1], a1, bf);
+            }
+        }
+        // ---- chain rule (eq. 6), lane-local
+        const int jj = pl ? j + Nt : j;
+        const double sp = p.sin_p[jj], cp = p.cos_p[jj];
+        const size_t fs = (size_t)p.nf * npts;
+#pragma unroll
+        for (int a = 0; a < 2; a++) {
+            const int irow = a ? ir1 : ir0;
+            if (irow >= Nt || (a && !r1ok)) continue;
+            const double st = p.sin_t[irow], ct = p.cos_t[irow], ist = p.inv_sin_t[irow];
+            const size_t base = (size_t)mu * npts + (size_t)jj * plane + (size_t)irow * Nr;
+#pragma unroll
+            for (int q = 0; q < GR_KT; q++) {
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    const int k = (kt0 + q) * 8 + 2 * t + e;
+                    if (k < Nr) {
+                        const double ir = p.inv_r[k];
+                        const double va = ar[a][q][e], vb = at[a][q][e] * ir, vc = p.dphi[base + k] * ir * ist;
+                        p.du[base + k] = st * cp * va + ct * cp * vb - sp * vc;
+                        p.du[fs + base + k] = st * sp * va + ct * sp * vb + cp * vc;
+                        p.du[2 * fs + base + k] = ct * va - st * vb;
+                    }
+                }
+            }
+        }
+    }
+}

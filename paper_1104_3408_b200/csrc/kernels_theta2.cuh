@@ -1,0 +1,157 @@
+// theta step of the Yn filter (eq. 61-62; 374-376), shared-memory staged.
+//   coef[dof][mc][i][k]  (mc = 0: a_0; 2m-1: a_m; 2m: b_m)  ->  cout, same layout
+// CTA = (component, m, block of 36 radii).  K (= latitude ii) is walked in chunks of 8 through a 4-stage
+// cp.async pipeline holding the F^n_m rows (and F^{-n}_m for complex components) and the raw coefficient
+// rows a_m, b_m (real) or a^r, b^r, a^i, b^i (complex) of the CTA's radii.
+// Warp (mg, ng): MT latitude tiles x 3 column tiles; a column tile is 4 radii x {v = 0, 1} interleaved
+// (col = 2k + v), so a lane's accumulator pair is the (v=0, v=1) pair of one radius:
+//   real (n = 0):  v=0: a~_m = F^0_m a_m,  v=1: b~_m = F^0_m b_m
+//   complex spin n, m > 0 (reading Q12, F^n_{-m} = F^{-n}_m by eq. 47):
+//       (p, q) = F^n_m    [(a^r + b^i)/2 , (a^i - b^r)/2]      = (Re, Im) c~_{+m}
+//       (s, t) = F^{-n}_m [(a^r - b^i)/2 , (a^i + b^r)/2]      = (Re, Im) c~_{-m}
+//       a~^r = p + s, b~^r = t - q, a~^i = q + t, b~^i = p - s
+//   complex, m = 0:  a~^r_0 = F^n_0 a^r_0, a~^i_0 = F^n_0 a^i_0.
+#pragma once
+#include "kernels_gemm2.cuh"
+
+#define TH_NT 3
+#define TH_NGC 3
+#define TH_RC (TH_NGC * TH_NT * 4)     // 36 radii per CTA
+#define TH_PKB 37
+#define TH_KC 8
+#define TH_STAGES 4
+#define TH_PA 12
+
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gmem));
+}
+
+struct ThetaComp2 { int dof; int n; };
+#define SP_THETA2_BATCH 96
+struct ThetaBatch2 { ThetaComp2 c[SP_THETA2_BATCH]; };
+
+// F2: [7][L+1][Nt8][Nt8] zero padded
+template <int MT, bool CPLX>
+__global__ void __launch_bounds__(512, 1)
+k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt8, int Nr, int MC4, int mgroups,
+         const double *__restrict__ coef, double *__restrict__ cout) {
+    extern __shared__ __align__(16) double sm[];
+    constexpr int NMAT = CPLX ? 2 : 1, NARR = CPLX ? 4 : 2;
+    const ThetaComp2 cmp = comps.c[blockIdx.y];
+    const int m = blockIdx.x;
+    const int k0 = blockIdx.z * TH_RC;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    const int mg = warp % mgroups, ng = warp / mgroups;
+    const size_t vec = (size_t)Nt * Nr, dofsz = (size_t)MC4 * vec, fsz = (size_t)Nt8 * Nt8;
+    const int mca = (m == 0) ? 0 : 2 * m - 1, mcb = 2 * m;
+    const int stageA = NMAT * Nt8 * TH_PA, stageB = NARR * TH_KC * TH_PKB;
+    double *As = sm, *Bs = sm + TH_STAGES * stageA;
+    const int nrad = min(TH_RC, Nr - k0);
+    // source arrays: real: [a_m, b_m]; complex: [a^r, b^r, a^i, b^i]
+    const double *srcR = coef + (size_t)cmp.dof * dofsz + k0;            // arr = 2*part + (0: a_m, 1: b_m)
+    const double *F0 = F2 + ((size_t)(3 + cmp.n) * (L + 1) + m) * fsz;
+    const long dF = CPLX ? -2L * cmp.n * (long)(L + 1) * (long)fsz : 0L;   // F^{-n}_m relative to F^n_m
+    const int nchunks = Nt8 / TH_KC;
+
+    auto load_chunk = [&](int kc, int st) {
+        double *as = As + st * stageA;
+        for (int q = tid; q < NMAT * Nt8 * 4; q += blockDim.x) {
+            const int mat = q / (Nt8 * 4), r = (q >> 2) % Nt8, h = q & 3;
+            cp_async16(as + (mat * Nt8 + r) * TH_PA + 2 * h, F0 + mat * dF + (size_t)r * Nt8 + kc * TH_KC + 2 * h);
+        }
+        double *bs = Bs + st * stageB;
+        for (int q = tid; q < NARR * TH_KC * TH_RC; q += blockDim.x) {
+            const int arr = q / (TH_KC * TH_RC), r = (q / TH_RC) % TH_KC, k = q % TH_RC;
+            const int ii = kc * TH_KC + r;
+            double *dst = bs + (arr * TH_KC + r) * TH_PKB + k;
+            const bool live = ii < Nt && k < nrad && !(m == 0 && (arr & 1));       // b_0 does not exist
+            if (live) cp_async8(dst, srcR + (size_t)(arr >> 1) * dofsz + (size_t)((arr & 1) ? mcb : mca) * vec + (size_t)ii * Nr + k);
+            else *dst = 0.0;
+        }
+    };
+
+    double acc[NMAT][MT][TH_NT][2];
+#pragma unroll
+    for (int x = 0; x < NMAT; x++)
+#pragma unroll
+        for (int a = 0; a < MT; a++)
+#pragma unroll
+            for (int b = 0; b < TH_NT; b++) acc[x][a][b][0] = acc[x][a][b][1] = 0.0;
+
+#pragma unroll
+    for (int s = 0; s < TH_STAGES - 1; s++) {
+        if (s < nchunks) load_chunk(s, s);
+        cp_async_commit();
+    }
+    const int v = g & 1, kq = g >> 1;
+    // B-fragment sources of this lane: real: arr v; complex: X = v ? a^i : a^r, Y = v ? b^r : b^i (sign -1 if v)
+    const int arrX = CPLX ? (v ? 2 : 0) : v, arrY = CPLX ? (v ? 1 : 3) : 0;
+    const double ysgn = v ? -0.5 : 0.5;
+    for (int kc = 0; kc < nchunks; kc++) {
+        cp_async_wait<TH_STAGES - 2>();
+        __syncthreads();
+        if (kc + TH_STAGES - 1 < nchunks) load_chunk(kc + TH_STAGES - 1, (kc + TH_STAGES - 1) % TH_STAGES);
+        cp_async_commit();
+        const double *as = As + (kc % TH_STAGES) * stageA + (mg * MT * 8 + g) * TH_PA + t;
+        const double *bs = Bs + (kc % TH_STAGES) * stageB;
+#pragma unroll
+        for (int ks = 0; ks < TH_KC / 4; ks++) {
+            double b1[TH_NT], b2[TH_NT];
+#pragma unroll
+            for (int b = 0; b < TH_NT; b++) {
+                const int kk = (ng * TH_NT + b) * 4 + kq;
+                const double x = bs[(arrX * TH_KC + ks * 4 + t) * TH_PKB + kk];
+                if (CPLX) {
+                    const double y = ysgn * bs[(arrY * TH_KC + ks * 4 + t) * TH_PKB + kk];
+                    b1[b] = (m > 0) ? 0.5 * x + y : x;
+                    b2[b] = 0.5 * x - y;
+                } else {
+                    b1[b] = x;
+                }
+            }
+#pragma unroll
+            for (int a = 0; a < MT; a++) {
+                const double a1 = as[a * 8 * TH_PA + ks * 4];
+#pragma unroll
+                for (int b = 0; b < TH_NT; b++) dmma(acc[0][a][b][0], acc[0][a][b][1], a1, b1[b]);
+                if (CPLX) {
+                    const double a2 = as[(Nt8 + a * 8) * TH_PA + ks * 4];
+#pragma unroll
+                    for (int b = 0; b < TH_NT; b++) dmma(acc[NMAT - 1][a][b][0], acc[NMAT - 1][a][b][1], a2, b2[b]);
+                }
+            }
+        }
+    }
+    // epilogue: lane owns latitude i = (mg*MT + a)*8 + g and radius k = k0 + (ng*3 + b)*4 + t
+    double *Ro = cout + (size_t)cmp.dof * dofsz, *Io = Ro + dofsz;
+#pragma unroll
+    for (int a = 0; a < MT; a++) {
+        const int i = (mg * MT + a) * 8 + g;
+        if (i >= Nt) continue;
+#pragma unroll
+        for (int b = 0; b < TH_NT; b++) {
+            const int kl = (ng * TH_NT + b) * 4 + t;
+            if (kl >= nrad) continue;
+            const size_t off = (size_t)i * Nr + k0 + kl;
+            const double pp = acc[0][a][b][0], qq = acc[0][a][b][1];
+            if (!CPLX) {
+                Ro[(size_t)mca * vec + off] = pp;
+                if (m > 0) Ro[(size_t)mcb * vec + off] = qq;
+            } else if (m > 0) {
+                const double ss = acc[NMAT - 1][a][b][0], tt = acc[NMAT - 1][a][b][1];
+                Ro[(size_t)mca * vec + off] = pp + ss;
+                Ro[(size_t)mcb * vec + off] = tt - qq;
+                Io[(size_t)mca * vec + off] = qq + tt;
+                Io[(size_t)mcb * vec + off] = pp - ss;
+            } else {
+                Ro[off] = pp;
+                Io[off] = qq;
+            }
+        }
+    }
+}
+
+static inline size_t theta2_smem_bytes(int Nt8, bool cplx) {
+    return (size_t)TH_STAGES * ((size_t)(cplx ? 2 : 1) * Nt8 * TH_PA + (cplx ? 4 : 2) * TH_KC * TH_PKB) * sizeof(double);
+}

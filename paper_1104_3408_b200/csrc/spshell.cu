@@ -111,12 +111,12 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
         if ((st = upload(&s->d_an, a.data(), a.size())) != SP_OK) return st;
         if ((st = upload(&s->d_sy, y.data(), y.size())) != SP_OK) return st;
     }
-    {   // F [7][L+1][Nt8][Nt4]
-        std::vector<double> f((size_t)7 * (L + 1) * s->Nt8 * s->Nt4, 0.0);
+    {   // F [7][L+1][Nt8][Nt8]
+        std::vector<double> f((size_t)7 * (L + 1) * s->Nt8 * s->Nt8, 0.0);
         for (int q = 0; q < 7 * (L + 1); q++)
             for (int i = 0; i < Nt; i++)
                 for (int j = 0; j < Nt; j++)
-                    f[((size_t)q * s->Nt8 + i) * s->Nt4 + j] = H.F[((size_t)q * Nt + i) * Nt + j];
+                    f[((size_t)q * s->Nt8 + i) * s->Nt8 + j] = H.F[((size_t)q * Nt + i) * Nt + j];
         if ((st = upload(&s->d_F, f.data(), f.size())) != SP_OK) return st;
     }
     {   // padded operands of k_phi_gemm
@@ -190,6 +190,7 @@ extern "C" sp_status sp_get_matrix(const sp_shell *s, int which, int n, int m, d
 #include "kernels_gemm.cuh"
 #include "kernels_grad.cuh"
 #include "kernels_filter.cuh"
+#include "kernels_theta2.cuh"
 #include "kernels_wave.cuh"
 
 static size_t grad_smem_bytes(const sp_shell *s) {
@@ -201,10 +202,24 @@ sp_status sp_configure_kernels(sp_shell *s) {
     if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;       // (r,theta) plane pair must fit one SM's shared memory
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     const int pg = (int)((size_t)PG_STAGES * ((size_t)4 * 6 * 8 * PG_PA + PG_KC * PG_PB) * sizeof(double));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    if (s->Nt8 / 8 <= 20) {
+        const int t1 = (int)theta2_smem_bytes(s->Nt8, false), t2 = (int)theta2_smem_bytes(s->Nt8, true);
+        if (t2 > 227 * 1024) return SP_ERR_UNSUPPORTED;
+        SP_CUDA(cudaFuncSetAttribute(k_theta2<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));
+        SP_CUDA(cudaFuncSetAttribute(k_theta2<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));
+        SP_CUDA(cudaFuncSetAttribute(k_theta2<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));
+        SP_CUDA(cudaFuncSetAttribute(k_theta2<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));
+        SP_CUDA(cudaFuncSetAttribute(k_theta2<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
+        SP_CUDA(cudaFuncSetAttribute(k_theta2<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
+        SP_CUDA(cudaFuncSetAttribute(k_theta2<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
+        SP_CUDA(cudaFuncSetAttribute(k_theta2<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
+    }
     return SP_OK;
 }
 
@@ -246,14 +261,10 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     const int itiles = s->Nt8 / 8, ktiles = s->Nr8 / 8;
     const size_t sm = grad_smem_bytes(s);
     dim3 grid(Nt, nf);
-    if (ktiles <= 3 || ktiles == 6 || ktiles == 9) {
-        int ntasks = 2 * itiles * ((ktiles + 2) / 3);
-        int nw = ntasks < 16 ? ntasks : 16;
-        k_grad_rtheta<3><<<grid, nw * 32, sm, st>>>(p);
-    } else {
-        int ntasks = 2 * itiles * ((ktiles + 4) / 5);
-        int nw = ntasks < 16 ? ntasks : 16;
-        k_grad_rtheta<5><<<grid, nw * 32, sm, st>>>(p);
+    {
+        const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + GR_KT - 1) / GR_KT);
+        const int nw = ntasks < 12 ? ntasks : 12;
+        k_grad_rtheta2<<<grid, nw * 32, sm, st>>>(p);
     }
     sp_mark(s, st, 2);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
@@ -373,7 +384,7 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     sp_mark(s, st, 3);
     for (int t = 0; t < ntens; t++) launch_pointwise<false>(types[t], targs[t], s, u, dofs, st);
     sp_mark(s, st, 4);
-    g_sp_launches += 2 * ntens + 2 + (comps.size() + SP_THETA_BATCH - 1) / SP_THETA_BATCH;
+    g_sp_launches += 2 * ntens + 2;
     // ---- F2: phi analysis (eq. 33)
     PhiTiling tla = {s->an_MT, s->an_mg, s->an_Mpad}, tls = {s->sy_MT, s->sy_mg, s->sy_Mpad};
     sp_status e = launch_phi_gemm(s->d_anp, s->Np8, s->MC, tla, Np, dofs, (long)vec, (long)npts, coef1, (long)vec, (long)(s->MC4 * vec),
@@ -385,18 +396,45 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     sp_mark(s, st, 5);
     // ---- F3: per-(n,m) theta matrices (eq. 62)
     {
-        const int nwarps = (Nr + 3) / 4, mtiles = s->Nt8 / 8;
-        for (size_t c0 = 0; c0 < comps.size(); c0 += SP_THETA_BATCH) {
-            ThetaBatch b;
-            int nb = (int)std::min<size_t>(SP_THETA_BATCH, comps.size() - c0);
-            for (int q = 0; q < nb; q++) b.c[q] = comps[c0 + q];
+        const int mtiles = s->Nt8 / 8;
+        const int MT = (mtiles % 3 == 0) ? 3 : (mtiles % 4 == 0) ? 4 : (mtiles < 3 ? mtiles : 3);
+        const int mgroups = (mtiles + MT - 1) / MT;
+        if (mgroups * TH_NGC <= 16) {
+            std::vector<ThetaComp2> rl, cx;
+            for (const ThetaComp &c : comps) (c.cplx ? cx : rl).push_back({c.dof, c.n});
+            const dim3 block(mgroups * TH_NGC * 32);
+            const int gz = (Nr + TH_RC - 1) / TH_RC;
+            for (int pass = 0; pass < 2; pass++) {
+                const std::vector<ThetaComp2> &lst = pass ? cx : rl;
+                const size_t sm = theta2_smem_bytes(s->Nt8, pass == 1);
+                for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
+                    ThetaBatch2 b;
+                    const int nb = (int)std::min<size_t>(SP_THETA2_BATCH, lst.size() - c0);
+                    for (int q = 0; q < nb; q++) b.c[q] = lst[c0 + q];
+                    const dim3 grid(s->L + 1, nb, gz);
+#define SP_TH2(MTV)                                                                                                          \
+    if (pass) k_theta2<MTV, true><<<grid, block, sm, st>>>(b, s->d_F, s->L, Nt, s->Nt8, Nr, s->MC4, mgroups, coef1, coef2);   \
+    else k_theta2<MTV, false><<<grid, block, sm, st>>>(b, s->d_F, s->L, Nt, s->Nt8, Nr, s->MC4, mgroups, coef1, coef2);
+                    switch (MT) {
+                        case 1: SP_TH2(1) break;
+                        case 2: SP_TH2(2) break;
+                        case 3: SP_TH2(3) break;
+                        default: SP_TH2(4) break;
+                    }
+#undef SP_TH2
+                    g_sp_launches += 1;
+                }
+            }
+        } else {   // very large Ntheta: generic global-memory kernel
+            const int nwarps = (Nr + 3) / 4;
             if (nwarps > 20) return SP_ERR_UNSUPPORTED;
-            if (mtiles % 3 == 0) {
-                dim3 grid(s->L + 1, nb, mtiles / 3);
-                k_theta<3><<<grid, nwarps * 32, 0, st>>>(b, s->d_F, s->L, Nt, s->Nt8, s->Nt4, Nr, s->MC4, coef1, coef2);
-            } else {
+            for (size_t c0 = 0; c0 < comps.size(); c0 += SP_THETA_BATCH) {
+                ThetaBatch b;
+                int nb = (int)std::min<size_t>(SP_THETA_BATCH, comps.size() - c0);
+                for (int q = 0; q < nb; q++) b.c[q] = comps[c0 + q];
                 dim3 grid(s->L + 1, nb, (mtiles + 3) / 4);
-                k_theta<4><<<grid, nwarps * 32, 0, st>>>(b, s->d_F, s->L, Nt, s->Nt8, s->Nt4, Nr, s->MC4, coef1, coef2);
+                k_theta<4><<<grid, nwarps * 32, 0, st>>>(b, s->d_F, s->L, Nt, s->Nt8, s->Nt8, Nr, s->MC4, coef1, coef2);
+                g_sp_launches += 1;
             }
         }
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
