@@ -123,108 +123,157 @@ __device__ __forceinline__ void cp_async8g(void *smem, const void *gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gmem));
 }
 
-#define GR_KT 3
-__global__ void __launch_bounds__(384, 2) k_grad_rtheta2(GradParams p) {
+// Preconditions (checked by the launcher, else the generic k_grad_rtheta runs): Ntheta % 4 == 0.
+// Layout of shared memory: P0, P1 [Nt8][PU] (PU >= padded column count, = 4 mod 8), CDs [NK8][PU] with
+// NK8 = kgroups*KT*8 rows, g2d [4 Nt + 8] = the circulant generator of FD_{2Nt} repeated twice.
+// Garbage in padded ROWS / COLUMNS of an operand only reaches discarded outputs (DMMA rows and columns are
+// independent); only the contraction padding (kk >= Nr) must be zero, and it is, in both operands.
+template <int KT>
+__global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_rtheta2(GradParams p) {
     extern __shared__ double sm[];
     const int Nr = p.Nr, Nt = p.Nt, Np = p.Np, PU = p.PU;
-    double *P0 = sm, *P1 = sm + (size_t)p.Nt8 * PU, *CDs = P1 + (size_t)p.Nt8 * PU, *g2s = CDs + (size_t)p.Nr8 * PU;
+    const int itiles = p.Nt8 >> 3, ipairs = (itiles + 1) >> 1, ktiles = p.Nr8 >> 3, kgroups = (ktiles + KT - 1) / KT;
+    const int NK8 = kgroups * KT * 8, n2 = 2 * Nt;
+    double *P0 = sm, *P1 = sm + (size_t)(p.Nt8 + 8) * PU, *CDs = P1 + (size_t)(p.Nt8 + 8) * PU, *g2d = CDs + (size_t)NK8 * PU;
+    double *tir = g2d + 2 * n2 + 8, *tst = tir + NK8, *tct = tst + p.Nt8 + 8, *tis = tct + p.Nt8 + 8;   // 1/r, sin, cos, 1/sin(theta)
     const int j = blockIdx.x, mu = blockIdx.y;
     const size_t npts = (size_t)Nr * Nt * Np, plane = (size_t)Nr * Nt;
     const double *u0 = p.u + mu * npts + (size_t)j * plane, *u1 = u0 + (size_t)Nt * plane;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
 
-    // planes: asynchronous 8-byte copies into the padded pitch
-    for (int q = threadIdx.x; q < Nt * Nr; q += blockDim.x) {
-        const int i = q / Nr, k = q - i * Nr;
-        cp_async8g(P0 + i * PU + k, u0 + q);
-        cp_async8g(P1 + i * PU + k, u1 + q);
+    // planes: one latitude row per warp iteration, 8-byte cp.async into the padded pitch; pad columns zeroed
+    for (int i = warp; i < p.Nt8 + 8; i += nwarps) {
+        for (int k = lane; k < PU; k += 32) {
+            if (i < Nt && k < Nr) {
+                cp_async8g(P0 + i * PU + k, u0 + (size_t)i * Nr + k);
+                cp_async8g(P1 + i * PU + k, u1 + (size_t)i * Nr + k);
+            } else {
+                P0[i * PU + k] = 0.0; P1[i * PU + k] = 0.0;
+            }
+        }
+    }
+    // CD^ rows (16-byte copies: the pitch PU is even), circulant table and Jacobian tables: all asynchronous,
+    // so the whole prologue costs one round trip to L2 instead of one per loop iteration
+    for (int q = threadIdx.x; q < NK8 * (PU / 2); q += blockDim.x) {
+        const int r = q / (PU / 2), h = q - r * (PU / 2);
+        if (r < p.Nr8) {
+            unsigned sa = (unsigned)__cvta_generic_to_shared(CDs + r * PU + 2 * h);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(p.cd + r * PU + 2 * h));
+        } else {
+            CDs[r * PU + 2 * h] = 0.0; CDs[r * PU + 2 * h + 1] = 0.0;
+        }
+    }
+    for (int q = threadIdx.x; q < 2 * n2 + 8; q += blockDim.x) cp_async8g(g2d + q, p.g2 + (q % n2));
+    for (int q = threadIdx.x; q < NK8; q += blockDim.x) {
+        if (q < Nr) cp_async8g(tir + q, p.inv_r + q); else tir[q] = 0.0;
+    }
+    for (int q = threadIdx.x; q < p.Nt8 + 8; q += blockDim.x) {
+        if (q < Nt) { cp_async8g(tst + q, p.sin_t + q); cp_async8g(tct + q, p.cos_t + q); cp_async8g(tis + q, p.inv_sin_t + q); }
+        else { tst[q] = 0.0; tct[q] = 0.0; tis[q] = 0.0; }
     }
     asm volatile("cp.async.commit_group;\n" ::);
-    // padding of the planes
-    const int padc = PU - Nr;
-    for (int q = threadIdx.x; q < Nt * padc; q += blockDim.x) {
-        const int i = q / padc, k = Nr + (q - i * padc);
-        P0[i * PU + k] = 0.0; P1[i * PU + k] = 0.0;
-    }
-    for (int q = threadIdx.x; q < (p.Nt8 - Nt) * PU; q += blockDim.x) { P0[Nt * PU + q] = 0.0; P1[Nt * PU + q] = 0.0; }
-    for (int q = threadIdx.x; q < p.Nr8 * PU; q += blockDim.x) CDs[q] = __ldg(p.cd + q);
-    for (int q = threadIdx.x; q < 2 * Nt; q += blockDim.x) g2s[q] = __ldg(p.g2 + q);
     asm volatile("cp.async.wait_group 0;\n" ::);
     __syncthreads();
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
     const int g = lane >> 2, t = lane & 3;
-    const int itiles = p.Nt8 >> 3, ipairs = (itiles + 1) >> 1, ktiles = p.Nr8 >> 3, kgroups = (ktiles + GR_KT - 1) / GR_KT;
     const int ntasks = 2 * ipairs * kgroups;
-    const int n2 = 2 * Nt;
     for (int task = warp; task < ntasks; task += nwarps) {
         const int pl = task / (ipairs * kgroups);
         const int rem = task - pl * ipairs * kgroups;
         const int ip = rem / kgroups, kg = rem - ip * kgroups;
         const double *Pown = pl ? P1 : P0, *Poth = pl ? P0 : P1;
-        const int kt0 = kg * GR_KT;
-        const int ir0 = ip * 16 + g, ir1 = ir0 + 8;          // the lane's two latitude rows
-        const bool r1ok = (ip * 2 + 1) < itiles;
-        double at[2][GR_KT][2], ar[2][GR_KT][2];
+        const int kt0 = kg * KT;
+        const int ir0 = ip * 16 + g, ir1 = ir0 + 8;          // the lane's two latitude rows (rows < Nt8 + 8 exist)
+        double at[2][KT][2], ar[2][KT][2];
 #pragma unroll
         for (int a = 0; a < 2; a++)
 #pragma unroll
-            for (int q = 0; q < GR_KT; q++) at[a][q][0] = at[a][q][1] = ar[a][q][0] = ar[a][q][1] = 0.0;
-        // ---- d/dtheta over the extended latitude index ii = 4 ks + t (eq. 8 with the double cover)
-        int d0 = ir0 - t; d0 += (d0 < 0) ? n2 : 0;
-        int d1 = ir1 - t; d1 += (d1 < 0) ? n2 : 0; d1 -= (d1 >= n2) ? n2 : 0;
-        const int ksteps = (n2 + 3) >> 2;
-        for (int ks = 0; ks < ksteps; ks++) {
-            const int ii = ks * 4 + t;
-            const bool iok = ii < n2;
-            const double a0 = (iok && ir0 < Nt) ? g2s[d0] : 0.0;
-            const double a1 = (iok && r1ok && ir1 < Nt) ? g2s[d1] : 0.0;
-            d0 -= 4; d0 += (d0 < 0) ? n2 : 0;
-            d1 -= 4; d1 += (d1 < 0) ? n2 : 0;
-            const int iic = iok ? ii : n2 - 1;
-            const double *rowp = ((iic < Nt) ? (Pown + iic * PU) : (Poth + (n2 - 1 - iic) * PU)) + kt0 * 8 + g;
+            for (int q = 0; q < KT; q++) at[a][q][0] = at[a][q][1] = ar[a][q][0] = ar[a][q][1] = 0.0;
+        // ---- d/dtheta (eq. 8 on the double cover): A[i][ii] = g2[(i - ii) mod 2Nt]
+        //      first half ii < Nt: rows of the own plane ascending; second half: rows of the antipodal plane descending
+        {
+            const double *ga0 = g2d + (ir0 - t + n2), *ga1 = ga0 + 8;      // index (i - ii) + 2Nt, ii = 4 ks + t
+            const double *bp = Pown + t * PU + kt0 * 8 + g;
+#pragma unroll 2
+            for (int ks = 0; ks < Nt / 4; ks++) {
+                const double a0 = ga0[-4 * ks], a1 = ga1[-4 * ks];
 #pragma unroll
-            for (int q = 0; q < GR_KT; q++) {
-                const double bf = (kt0 + q < ktiles) ? rowp[q * 8] : 0.0;
-                dmma(at[0][q][0], at[0][q][1], a0, bf);
-                dmma(at[1][q][0], at[1][q][1], a1, bf);
+                for (int q = 0; q < KT; q++) {
+                    const double bf = bp[(size_t)ks * 4 * PU + q * 8];
+                    dmma(at[0][q][0], at[0][q][1], a0, bf);
+                    dmma(at[1][q][0], at[1][q][1], a1, bf);
+                }
+            }
+            ga0 -= Nt; ga1 -= Nt;
+            bp = Poth + (Nt - 1 - t) * PU + kt0 * 8 + g;                    // ii = Nt + 4 ks + t  ->  row 2Nt-1-ii
+#pragma unroll 2
+            for (int ks = 0; ks < Nt / 4; ks++) {
+                const double a0 = ga0[-4 * ks], a1 = ga1[-4 * ks];
+#pragma unroll
+                for (int q = 0; q < KT; q++) {
+                    const double bf = bp[-(ptrdiff_t)ks * 4 * PU + q * 8];
+                    dmma(at[0][q][0], at[0][q][1], a0, bf);
+                    dmma(at[1][q][0], at[1][q][1], a1, bf);
+                }
             }
         }
-        // ---- d/dr: A = u[i][kk], B[kk][k'] = CD^[k'][kk]   (eq. 9, 13)
-        const double *arow0 = Pown + ir0 * PU + t, *arow1 = Pown + (r1ok ? ir1 : ir0) * PU + t;
-        const double *cdp = CDs + (kt0 * 8 + g) * PU + t;
-        for (int ks = 0; ks < p.Nr4 / 4; ks++) {
-            const double a0 = arow0[ks * 4], a1 = arow1[ks * 4];
+        // d/dphi of the lane's outputs: prefetched into L1 now, read after the d/dr loop (hides the global latency)
+        const int jj = pl ? j + Nt : j;
+        const size_t pbase = (size_t)mu * npts + (size_t)jj * plane;
 #pragma unroll
-            for (int q = 0; q < GR_KT; q++) {
-                const double bf = (kt0 + q < ktiles) ? cdp[q * 8 * PU + ks * 4] : 0.0;
-                dmma(ar[0][q][0], ar[0][q][1], a0, bf);
-                dmma(ar[1][q][0], ar[1][q][1], a1, bf);
+        for (int a = 0; a < 2; a++) {
+            const int irow = a ? ir1 : ir0;
+#pragma unroll
+            for (int q = 0; q < KT; q++) {
+                const int k = (kt0 + q) * 8 + 2 * t;
+                if (irow < Nt && k < Nr) asm volatile("prefetch.global.L1 [%0];\n" ::"l"(p.dphi + pbase + (size_t)irow * Nr + k));
+            }
+        }
+        const double sp = __ldg(p.sin_p + jj), cp = __ldg(p.cos_p + jj);
+        // ---- d/dr: A = u[i][kk], B[kk][k'] = CD^[k'][kk]   (eq. 9, 13)
+        {
+            const double *arow0 = Pown + ir0 * PU + t, *arow1 = arow0 + 8 * PU;
+            const double *cdp = CDs + (kt0 * 8 + g) * PU + t;
+#pragma unroll 3
+            for (int ks = 0; ks < p.Nr4 / 4; ks++) {
+                const double a0 = arow0[ks * 4], a1 = arow1[ks * 4];
+#pragma unroll
+                for (int q = 0; q < KT; q++) {
+                    const double bf = cdp[q * 8 * PU + ks * 4];
+                    dmma(ar[0][q][0], ar[0][q][1], a0, bf);
+                    dmma(ar[1][q][0], ar[1][q][1], a1, bf);
+                }
             }
         }
         // ---- chain rule (eq. 6), lane-local
-        const int jj = pl ? j + Nt : j;
-        const double sp = p.sin_p[jj], cp = p.cos_p[jj];
         const size_t fs = (size_t)p.nf * npts;
 #pragma unroll
         for (int a = 0; a < 2; a++) {
             const int irow = a ? ir1 : ir0;
-            if (irow >= Nt || (a && !r1ok)) continue;
-            const double st = p.sin_t[irow], ct = p.cos_t[irow], ist = p.inv_sin_t[irow];
-            const size_t base = (size_t)mu * npts + (size_t)jj * plane + (size_t)irow * Nr;
+            if (irow >= Nt) continue;
+            const double st = tst[irow], ct = tct[irow], ist = tis[irow];
+            const double xa = st * cp, xb = ct * cp, ya = st * sp, yb = ct * sp;
+            const size_t base = pbase + (size_t)irow * Nr;
 #pragma unroll
-            for (int q = 0; q < GR_KT; q++) {
+            for (int q = 0; q < KT; q++) {
 #pragma unroll
                 for (int e = 0; e < 2; e++) {
                     const int k = (kt0 + q) * 8 + 2 * t + e;
                     if (k < Nr) {
-                        const double ir = p.inv_r[k];
-                        const double va = ar[a][q][e], vb = at[a][q][e] * ir, vc = p.dphi[base + k] * ir * ist;
-                        p.du[base + k] = st * cp * va + ct * cp * vb - sp * vc;
-                        p.du[fs + base + k] = st * sp * va + ct * sp * vb + cp * vc;
+                        const double ir = tir[k];
+                        const double va = ar[a][q][e], vb = at[a][q][e] * ir, vc = __ldg(p.dphi + base + k) * (ir * ist);
+                        p.du[base + k] = xa * va + xb * vb - sp * vc;
+                        p.du[fs + base + k] = ya * va + yb * vb + cp * vc;
                         p.du[2 * fs + base + k] = ct * va - st * vb;
                     }
                 }
             }
         }
     }
+}
+
+// shared memory of k_grad_rtheta2<KT>
+static inline size_t grad2_smem_bytes(int Nt, int Nt8, int Nr8, int PU, int KT) {
+    const int ktiles = Nr8 / 8, NK8 = ((ktiles + KT - 1) / KT) * KT * 8;
+    return ((size_t)2 * (Nt8 + 8) * PU + (size_t)NK8 * PU + 4 * Nt + 8 + NK8 + 3 * (Nt8 + 8)) * sizeof(double);
 }

@@ -9,6 +9,7 @@ struct sp_shell {
     int Nr, Nt, Np, L;
     double rin, rout;
     int Nr8, Nr4, Nt8, Nt4, MC, MC4, MC8, J8, PU;
+    int gradKT;                   // radial tiles per warp task of k_grad_rtheta2 (3 or 5)
     size_t npts;
     bool built, host_built;
     SpHostMatrices *host = nullptr;

@@ -47,7 +47,11 @@ extern "C" sp_status sp_shell_create(int Nr, int Nt, int Np, double rin, double 
     s->Nt8 = round_up(Nt, 8); s->Nt4 = round_up(Nt, 4);
     s->MC = 2 * L + 1; s->MC4 = round_up(s->MC, 4); s->MC8 = round_up(s->MC, 8);
     s->J8 = round_up(Np, 8);
-    s->PU = s->Nr8 + 4;                                                       // smem pitch == 4 (mod 8): conflict-free fragments
+    {   // radial tiling of the (r,theta) kernel and the shared-memory pitch (= 4 mod 8: conflict-free fragments)
+        const int ktiles = s->Nr8 / 8;
+        s->gradKT = (ktiles % 3 != 0 && ktiles % 5 == 0) ? 5 : 3;
+        s->PU = (ktiles + s->gradKT - 1) / s->gradKT * s->gradKT * 8 + 4;
+    }
     s->npts = (size_t)Nr * Nt * Np;
     s->built = false; s->host_built = false;
     *out = s;
@@ -202,8 +206,12 @@ sp_status sp_configure_kernels(sp_shell *s) {
     if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;       // (r,theta) plane pair must fit one SM's shared memory
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    const size_t sm2 = grad2_smem_bytes(s->Nt, s->Nt8, s->Nr8, s->PU, s->gradKT);
+    if (sm2 > 227 * 1024) return SP_ERR_UNSUPPORTED;
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     const int pg = (int)((size_t)PG_STAGES * ((size_t)4 * 6 * 8 * PG_PA + PG_KC * PG_PB) * sizeof(double));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
@@ -261,10 +269,15 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     const int itiles = s->Nt8 / 8, ktiles = s->Nr8 / 8;
     const size_t sm = grad_smem_bytes(s);
     dim3 grid(Nt, nf);
-    {
-        const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + GR_KT - 1) / GR_KT);
-        const int nw = ntasks < 12 ? ntasks : 12;
-        k_grad_rtheta2<<<grid, nw * 32, sm, st>>>(p);
+    if (Nt % 4 == 0) {
+        const int KT = s->gradKT;
+        const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
+        const size_t sm2 = grad2_smem_bytes(Nt, s->Nt8, s->Nr8, s->PU, KT);
+        if (KT == 3) k_grad_rtheta2<3><<<grid, (ntasks < 12 ? ntasks : 12) * 32, sm2, st>>>(p);
+        else k_grad_rtheta2<5><<<grid, (ntasks < 6 ? ntasks : 6) * 32, sm2, st>>>(p);
+    } else {   // Ntheta not a multiple of 4: generic kernel
+        const int ntasks = 2 * itiles * ((ktiles + 4) / 5);
+        k_grad_rtheta<5><<<grid, (ntasks < 16 ? ntasks : 16) * 32, sm, st>>>(p);
     }
     sp_mark(s, st, 2);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
