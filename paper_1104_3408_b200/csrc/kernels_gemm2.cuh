@@ -24,13 +24,25 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
-template <int MT>
+// EPI_GRAD: gradient epilogue (eq. 6).  The product is d/dphi u (A = FD_{Nphi}); C holds on entry the
+// phi-independent combination W written by k_grad_rtheta2<.., SPLIT> and receives d_x u; Y receives d_y u:
+//     c = (d_phi u)/(r sin th),   d_x = cos(ph) W - sin(ph) c,   d_y = sin(ph) W + cos(ph) c.
+// The CTA's W tile [M][64] is fetched by cp.async at kernel start into its own shared-memory tile (pitch 72).
+struct PhiGradEpi {
+    double *Y; long sYb;                      // d_y output, batch stride
+    const double *inv_r, *inv_sin_t, *sin_p, *cos_p;
+    int Nr;
+};
+#define PG_PW 72
+
+template <int MT, bool EPI_GRAD>
 __global__ void __launch_bounds__(512)
 k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const double *__restrict__ B, long sBk, long sBb,
-           double *__restrict__ C, long sCm, long sCb, int ncols) {
+           double *__restrict__ C, long sCm, long sCb, int ncols, PhiGradEpi ge) {
     extern __shared__ __align__(16) double sm[];
     const int stageA = Mpad * PG_PA, stageB = PG_KC * PG_PB;
     double *As = sm, *Bs = sm + PG_STAGES * stageA;
+    double *Ws = Bs + PG_STAGES * stageB;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp >> 2, ng = warp & 3;
     const int c0 = blockIdx.x * PG_NCOL;
@@ -63,6 +75,13 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
 #pragma unroll
         for (int b = 0; b < 2; b++) acc[a][b][0] = acc[a][b][1] = 0.0;
 
+    if (EPI_GRAD) {      // oldest cp.async group: complete long before the epilogue
+        for (int q = tid; q < M * (PG_NCOL / 2); q += blockDim.x) {
+            const int r = q >> 5, h = q & 31;
+            if (2 * h < colsleft) cp_async16(Ws + r * PG_PW + 2 * h, Cb + (long)r * sCm + 2 * h);
+        }
+        cp_async_commit();
+    }
 #pragma unroll
     for (int s = 0; s < PG_STAGES - 1; s++) {
         if (s < nchunks) load_chunk(s, s);
@@ -89,14 +108,45 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
             }
         }
     }
+    if (!EPI_GRAD) {
 #pragma unroll
-    for (int a = 0; a < MT; a++) {
-        const int row = (mg * MT + a) * 8 + g;
-        if (row >= M) continue;
+        for (int a = 0; a < MT; a++) {
+            const int row = (mg * MT + a) * 8 + g;
+            if (row >= M) continue;
 #pragma unroll
-        for (int b = 0; b < 2; b++) {
-            const int col = ng * 16 + b * 8 + 2 * t;
-            if (col < colsleft) *reinterpret_cast<double2 *>(Cb + (long)row * sCm + col) = make_double2(acc[a][b][0], acc[a][b][1]);
+            for (int b = 0; b < 2; b++) {
+                const int col = ng * 16 + b * 8 + 2 * t;
+                if (col < colsleft) *reinterpret_cast<double2 *>(Cb + (long)row * sCm + col) = make_double2(acc[a][b][0], acc[a][b][1]);
+            }
+        }
+    } else {
+        cp_async_wait<0>();
+        __syncthreads();                       // W tile (copied by all threads) visible to all
+        double *Yb = ge.Y + (long)blockIdx.y * ge.sYb + c0;
+        double f[2][2];                        // 1/(r sin th) of the lane's four columns
+#pragma unroll
+        for (int b = 0; b < 2; b++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const int c = c0 + ng * 16 + b * 8 + 2 * t + e;        // flat (k, i) column: c = k + Nr i
+                const int i = c / ge.Nr, k = c - i * ge.Nr;
+                f[b][e] = (c < ncols) ? __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i) : 0.0;
+            }
+#pragma unroll
+        for (int a = 0; a < MT; a++) {
+            const int row = (mg * MT + a) * 8 + g;                       // longitude j
+            if (row >= M) continue;
+            const double sp = __ldg(ge.sin_p + row), cp = __ldg(ge.cos_p + row);
+#pragma unroll
+            for (int b = 0; b < 2; b++) {
+                const int col = ng * 16 + b * 8 + 2 * t;
+                if (col < colsleft) {
+                    const double2 w = *reinterpret_cast<const double2 *>(Ws + row * PG_PW + col);
+                    const double ca = acc[a][b][0] * f[b][0], cb = acc[a][b][1] * f[b][1];
+                    *reinterpret_cast<double2 *>(Cb + (long)row * sCm + col) = make_double2(cp * w.x - sp * ca, cp * w.y - sp * cb);
+                    *reinterpret_cast<double2 *>(Yb + (long)row * sCm + col) = make_double2(sp * w.x + cp * ca, sp * w.y + cp * cb);
+                }
+            }
         }
     }
 }
@@ -115,22 +165,35 @@ static inline PhiTiling phi_tiling(int M) {
     best.Mpad = best.mgroups * best.MT * 8;
     return best;
 }
-static inline size_t phi_smem_bytes(const PhiTiling &tl) {
-    return (size_t)PG_STAGES * ((size_t)tl.Mpad * PG_PA + PG_KC * PG_PB) * sizeof(double);
+static inline size_t phi_smem_bytes(const PhiTiling &tl, int Mgrad = 0) {
+    return ((size_t)PG_STAGES * ((size_t)tl.Mpad * PG_PA + PG_KC * PG_PB) + (size_t)Mgrad * PG_PW) * sizeof(double);
 }
 
 // returns SP_ERR_UNSUPPORTED when the fast-path preconditions do not hold (caller falls back)
 static sp_status launch_phi_gemm(const double *A, int lda, int M, const PhiTiling &tl, int K, const double *B, long sBk, long sBb,
-                                 double *C, long sCm, long sCb, int ncols, int nbatch, cudaStream_t st) {
+                                 double *C, long sCm, long sCb, int ncols, int nbatch, cudaStream_t st,
+                                 const PhiGradEpi *ge = nullptr) {
     if ((sBk | sBb | sCm | sCb | (long)ncols) & 1) return SP_ERR_UNSUPPORTED;
     if (((uintptr_t)B | (uintptr_t)C) & 15) return SP_ERR_UNSUPPORTED;
     if (tl.mgroups > 4) return SP_ERR_UNSUPPORTED;
     dim3 grid((ncols + PG_NCOL - 1) / PG_NCOL, nbatch), block(tl.mgroups * 4 * 32);
+    if (ge) {
+        if ((ge->sYb & 1) || ((uintptr_t)ge->Y & 15)) return SP_ERR_UNSUPPORTED;
+        const size_t sm = phi_smem_bytes(tl, M);
+        if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;
+        switch (tl.MT) {
+            case 4: k_phi_gemm<4, true><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, *ge); break;
+            case 5: k_phi_gemm<5, true><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, *ge); break;
+            default: k_phi_gemm<6, true><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, *ge); break;
+        }
+        return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+    }
     const size_t sm = phi_smem_bytes(tl);
+    PhiGradEpi none = {};
     switch (tl.MT) {
-        case 4: k_phi_gemm<4><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols); break;
-        case 5: k_phi_gemm<5><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols); break;
-        default: k_phi_gemm<6><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols); break;
+        case 4: k_phi_gemm<4, false><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, none); break;
+        case 5: k_phi_gemm<5, false><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, none); break;
+        default: k_phi_gemm<6, false><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, none); break;
     }
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }

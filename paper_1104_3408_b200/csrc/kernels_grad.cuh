@@ -128,7 +128,12 @@ __device__ __forceinline__ void cp_async8g(void *smem, const void *gmem) {
 // NK8 = kgroups*KT*8 rows, g2d [4 Nt + 8] = the circulant generator of FD_{2Nt} repeated twice.
 // Garbage in padded ROWS / COLUMNS of an operand only reaches discarded outputs (DMMA rows and columns are
 // independent); only the contraction padding (kk >= Nr) must be zero, and it is, in both operands.
-template <int KT>
+// SPLIT = true: the kernel runs FIRST and writes the phi-independent combinations
+//     W = sin(th) d_r u + (cos(th)/r) d_th u  -> du[0] (x slot),     d_z u = cos(th) d_r u - (sin(th)/r) d_th u -> du[2];
+// the d/dphi GEMM that follows (k_phi_gemm<.., EPI_GRAD>) finishes d_x = cos(ph) W - sin(ph) c, d_y = sin(ph) W + cos(ph) c
+// with c = d_phi u /(r sin th) in its epilogue.  No global read sits on this kernel's critical path.
+// SPLIT = false: d/dphi is read from p.dphi and all three components are finished here.
+template <int KT, bool SPLIT>
 __global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_rtheta2(GradParams p) {
     extern __shared__ double sm[];
     const int Nr = p.Nr, Nt = p.Nt, Np = p.Np, PU = p.PU;
@@ -226,10 +231,10 @@ __global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_r
 #pragma unroll
             for (int q = 0; q < KT; q++) {
                 const int k = (kt0 + q) * 8 + 2 * t;
-                if (irow < Nt && k < Nr) asm volatile("prefetch.global.L1 [%0];\n" ::"l"(p.dphi + pbase + (size_t)irow * Nr + k));
+                if (!SPLIT && irow < Nt && k < Nr) asm volatile("prefetch.global.L1 [%0];\n" ::"l"(p.dphi + pbase + (size_t)irow * Nr + k));
             }
         }
-        const double sp = __ldg(p.sin_p + jj), cp = __ldg(p.cos_p + jj);
+        const double sp = SPLIT ? 0.0 : __ldg(p.sin_p + jj), cp = SPLIT ? 1.0 : __ldg(p.cos_p + jj);
         // ---- d/dr: A = u[i][kk], B[kk][k'] = CD^[k'][kk]   (eq. 9, 13)
         {
             const double *arow0 = Pown + ir0 * PU + t, *arow1 = arow0 + 8 * PU;
@@ -261,10 +266,16 @@ __global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_r
                     const int k = (kt0 + q) * 8 + 2 * t + e;
                     if (k < Nr) {
                         const double ir = tir[k];
-                        const double va = ar[a][q][e], vb = at[a][q][e] * ir, vc = __ldg(p.dphi + base + k) * (ir * ist);
-                        p.du[base + k] = xa * va + xb * vb - sp * vc;
-                        p.du[fs + base + k] = ya * va + yb * vb + cp * vc;
-                        p.du[2 * fs + base + k] = ct * va - st * vb;
+                        const double va = ar[a][q][e], vb = at[a][q][e] * ir;
+                        if (SPLIT) {
+                            p.du[base + k] = st * va + ct * vb;
+                            p.du[2 * fs + base + k] = ct * va - st * vb;
+                        } else {
+                            const double vc = __ldg(p.dphi + base + k) * (ir * ist);
+                            p.du[base + k] = xa * va + xb * vb - sp * vc;
+                            p.du[fs + base + k] = ya * va + yb * vb + cp * vc;
+                            p.du[2 * fs + base + k] = ct * va - st * vb;
+                        }
                     }
                 }
             }

@@ -9,6 +9,7 @@ struct sp_shell {
     int Nr, Nt, Np, L;
     double rin, rout;
     int Nr8, Nr4, Nt8, Nt4, MC, MC4, MC8, J8, PU;
+    bool grad_split_ok = false;   // the split gradient (r-theta kernel first, d/dphi GEMM with fused chain rule) is usable
     int gradKT;                   // radial tiles per warp task of k_grad_rtheta2 (3 or 5)
     size_t npts;
     bool built, host_built;
@@ -30,6 +31,7 @@ struct sp_shell {
     mutable bool prof = false;
     mutable cudaEvent_t ev[9] = {};
     mutable bool ev_set[9] = {};
+    mutable bool grad_swapped = false;   // last gradient ran (r,theta) kernel first, then the d/dphi GEMM
 };
 
 // stage marks: 0 grad start, 1 after d/dphi, 2 after r-theta+chain rule, 3 filter start, 4 after projection,

@@ -10,6 +10,7 @@
 
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 
 #define SP_CUDA(x)                                   \
@@ -50,6 +51,7 @@ extern "C" sp_status sp_shell_create(int Nr, int Nt, int Np, double rin, double 
     {   // radial tiling of the (r,theta) kernel and the shared-memory pitch (= 4 mod 8: conflict-free fragments)
         const int ktiles = s->Nr8 / 8;
         s->gradKT = (ktiles % 3 != 0 && ktiles % 5 == 0) ? 5 : 3;
+        if (const char *e = getenv("SP_GRAD_KT")) { if (atoi(e) == 3 || atoi(e) == 5) s->gradKT = atoi(e); }   // tuning override
         s->PU = (ktiles + s->gradKT - 1) / s->gradKT * s->gradKT * 8 + 4;
     }
     s->npts = (size_t)Nr * Nt * Np;
@@ -208,14 +210,26 @@ sp_status sp_configure_kernels(sp_shell *s) {
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const size_t sm2 = grad2_smem_bytes(s->Nt, s->Nt8, s->Nr8, s->PU, s->gradKT);
     if (sm2 > 227 * 1024) return SP_ERR_UNSUPPORTED;
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     const int pg = (int)((size_t)PG_STAGES * ((size_t)4 * 6 * 8 * PG_PA + PG_KC * PG_PB) * sizeof(double));
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    {
+        PhiTiling tg = phi_tiling(s->Np);
+        const size_t pgg = phi_smem_bytes(tg, s->Np);
+        s->grad_split_ok = pgg <= 227 * 1024 && tg.mgroups <= 4;
+        if (s->grad_split_ok) {
+            SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
+            SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
+            SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
+        }
+    }
     if (s->Nt8 / 8 <= 20) {
         const int t1 = (int)theta2_smem_bytes(s->Nt8, false), t2 = (int)theta2_smem_bytes(s->Nt8, true);
         if (t2 > 227 * 1024) return SP_ERR_UNSUPPORTED;
@@ -250,34 +264,54 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     cudaStream_t st = (cudaStream_t)stream;
     const int Nr = s->Nr, Nt = s->Nt, Np = s->Np;
     const long plane = (long)Nr * Nt;
-    double *dphi = (double *)ws;
-    sp_mark(s, st, 0);
-    // d/dphi: FD_{Np} (circulant) over j, stride Nr*Nt; every field is one batch          (eq. 8, 18)
-    PhiTiling tl = {s->fd3_MT, s->fd3_mg, s->fd3_Mpad};
-    sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
-    if (e == SP_ERR_UNSUPPORTED)   // odd strides: generic global-memory kernel
-        e = launch_gemm_cols<true>(s->d_g3, Np, Np, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
-    if (e != SP_OK) return e;
-    sp_mark(s, st, 1);
-    g_sp_launches += 2;
+    const int itiles = s->Nt8 / 8, ktiles = s->Nr8 / 8;
     GradParams p;
     p.Nr = Nr; p.Nt = Nt; p.Np = Np; p.PU = s->PU; p.Nr8 = s->Nr8; p.Nr4 = s->Nr4; p.Nt8 = s->Nt8;
     p.cd = s->d_cd; p.g2 = s->d_g2;
     p.inv_r = s->d_inv_r; p.sin_t = s->d_sin_t; p.cos_t = s->d_cos_t; p.inv_sin_t = s->d_inv_sin_t;
     p.sin_p = s->d_sin_p; p.cos_p = s->d_cos_p;
-    p.u = u; p.dphi = dphi; p.du = du; p.nf = nf;
-    const int itiles = s->Nt8 / 8, ktiles = s->Nr8 / 8;
-    const size_t sm = grad_smem_bytes(s);
-    dim3 grid(Nt, nf);
+    p.u = u; p.dphi = nullptr; p.du = du; p.nf = nf;
+    const dim3 grid(Nt, nf);
+    PhiTiling tl = {s->fd3_MT, s->fd3_mg, s->fd3_Mpad};
+    g_sp_launches += 2;
+    sp_mark(s, st, 0);
+    // ---- fast path: (r,theta)-plane kernel first (W -> du[x], d_z -> du[z]), then the d/dphi GEMM whose epilogue
+    //      applies the chain rule (eq. 6).  Needs Ntheta % 4 == 0, even strides and 16-byte aligned buffers.
+    const bool aligned = !(((uintptr_t)u | (uintptr_t)du) & 15) && !((plane | (long)s->npts) & 1);
+    if (Nt % 4 == 0 && s->grad_split_ok && aligned) {
+        const int KT = s->gradKT;
+        const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
+        const size_t sm2 = grad2_smem_bytes(Nt, s->Nt8, s->Nr8, s->PU, KT);
+        if (KT == 3) k_grad_rtheta2<3, true><<<grid, (ntasks < 12 ? ntasks : 12) * 32, sm2, st>>>(p);
+        else k_grad_rtheta2<5, true><<<grid, (ntasks < 6 ? ntasks : 6) * 32, sm2, st>>>(p);
+        if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
+        sp_mark(s, st, 1);
+        PhiGradEpi ge = {du + (size_t)nf * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
+        sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, du, plane, (long)s->npts, (int)plane, nf,
+                                      st, &ge);
+        if (e != SP_OK) return e;
+        sp_mark(s, st, 2);
+        s->grad_swapped = true;
+        return SP_OK;
+    }
+    // ---- general path: d/dphi into the workspace, then the plane kernel finishes all three components
+    s->grad_swapped = false;
+    double *dphi = (double *)ws;
+    p.dphi = dphi;
+    sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
+    if (e == SP_ERR_UNSUPPORTED)   // odd strides: generic global-memory kernel
+        e = launch_gemm_cols<true>(s->d_g3, Np, Np, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
+    if (e != SP_OK) return e;
+    sp_mark(s, st, 1);
     if (Nt % 4 == 0) {
         const int KT = s->gradKT;
         const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
         const size_t sm2 = grad2_smem_bytes(Nt, s->Nt8, s->Nr8, s->PU, KT);
-        if (KT == 3) k_grad_rtheta2<3><<<grid, (ntasks < 12 ? ntasks : 12) * 32, sm2, st>>>(p);
-        else k_grad_rtheta2<5><<<grid, (ntasks < 6 ? ntasks : 6) * 32, sm2, st>>>(p);
+        if (KT == 3) k_grad_rtheta2<3, false><<<grid, (ntasks < 12 ? ntasks : 12) * 32, sm2, st>>>(p);
+        else k_grad_rtheta2<5, false><<<grid, (ntasks < 6 ? ntasks : 6) * 32, sm2, st>>>(p);
     } else {   // Ntheta not a multiple of 4: generic kernel
         const int ntasks = 2 * itiles * ((ktiles + 4) / 5);
-        k_grad_rtheta<5><<<grid, (ntasks < 16 ? ntasks : 16) * 32, sm, st>>>(p);
+        k_grad_rtheta<5><<<grid, (ntasks < 16 ? ntasks : 16) * 32, grad_smem_bytes(s), st>>>(p);
     }
     sp_mark(s, st, 2);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
@@ -531,7 +565,8 @@ extern "C" sp_status sp_profile_enable(sp_shell *s, int on) {
 
 extern "C" sp_status sp_profile_read(const sp_shell *s, double *ms7) {
     if (!s || !ms7) return SP_ERR_INVALID_ARG;
-    static const int a[7] = {0, 1, 3, 4, 5, 6, 7}, b[7] = {1, 2, 4, 5, 6, 7, 8};
+    int a[7] = {0, 1, 3, 4, 5, 6, 7}, b[7] = {1, 2, 4, 5, 6, 7, 8};
+    if (s->grad_swapped) { a[0] = 1; b[0] = 2; a[1] = 0; b[1] = 1; }      // (r,theta) kernel ran first
     for (int q = 0; q < 7; q++) {
         ms7[q] = -1.0;
         if (s->ev_set[a[q]] && s->ev_set[b[q]]) {
