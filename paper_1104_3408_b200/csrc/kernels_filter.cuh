@@ -207,28 +207,76 @@ __device__ __forceinline__ void tensor_transform(const Trig &q, const double *in
 }
 
 // pointwise: INV = false: state fields -> dof arrays; INV = true: dof arrays -> state fields
+// pointwise, with the phi-reflection fold fused in.  The real Fourier transforms (eq. 20-24) see a function only
+// through E_j = f_j + f_{J-j} (cosine rows) and O_j = f_j - f_{J-j} (sine rows), j = 1..J/2-1, plus f_0 and f_{J/2}:
+//     a_m = (2/J) [ f_0 + (-1)^m f_{J/2} + sum_{j=1}^{J/2-1} cos(m phi_j) E_j ],   b_m = (2/J) sum_{j=1}^{J/2-1} sin(m phi_j) O_j,
+// which halves the contraction length of the analysis and synthesis products (same sums, regrouped).
+// Folded dof arrays [dof][row][i][k]: rows 0..J/2 hold f_0, E_1..E_{J/2-1}, f_{J/2}; rows J/2+j hold O_j.
+// One thread owns the grid points (k, i, j) and (k, i, J-j), j = 0..J/2.
+//   INV = false: state fields -> folded dofs;   INV = true: folded dofs -> state fields.
 template <int TT, bool INV>
 __global__ void __launch_bounds__(128)
 k_pointwise(TensorArgs ta, int Nr, int Nt, size_t npts, const double *__restrict__ sin_t, const double *__restrict__ cos_t,
             const double *__restrict__ sin_p, const double *__restrict__ cos_p, const double *src, double *dst) {
     constexpr int nc = TTInfo<TT>::nc;
-    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= npts) return;
-    const int i = (int)((p / Nr) % Nt), j = (int)(p / ((size_t)Nr * Nt));
-    Trig q = {sin_t[i], cos_t[i], sin_p[j], cos_p[j]};
-    double in[nc], out[nc];
+    const size_t plane = (size_t)Nr * Nt;
+    const size_t q0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;       // (k, i, j) with j in [0, J/2]
+    if (q0 >= plane * (size_t)(Nt + 1)) return;
+    const int j = (int)(q0 / plane);
+    const size_t ki = q0 - (size_t)j * plane;
+    const int i = (int)(ki / Nr);
+    const int J = 2 * Nt, j2 = J - j;
+    const bool paired = (j != 0) && (j != Nt);
+    const size_t p1 = (size_t)j * plane + ki, p2 = (size_t)j2 * plane + ki;   // the two grid points
+    const size_t pe = p1, po = (size_t)(Nt + j) * plane + ki;                // folded rows E_j and O_j
+    const double st = sin_t[i], ct = cos_t[i];
+    const Trig t1 = {st, ct, sin_p[j], cos_p[j]};
+    double a[nc], b[nc];
+    if (!INV) {
+        double in[nc];
 #pragma unroll
-    for (int c = 0; c < nc; c++) in[c] = INV ? src[(size_t)(ta.dof0 + c) * npts + p] : src[(size_t)ta.field[c] * npts + p];
-    tensor_transform<TT, INV>(q, in, out);
+        for (int c = 0; c < nc; c++) in[c] = src[(size_t)ta.field[c] * npts + p1];
+        tensor_transform<TT, false>(t1, in, a);
+        if (paired) {
+            const Trig t2 = {st, ct, sin_p[j2], cos_p[j2]};
 #pragma unroll
-    for (int c = 0; c < nc; c++) {
-        if (INV) dst[(size_t)ta.field[c] * npts + p] = out[c];
-        else dst[(size_t)(ta.dof0 + c) * npts + p] = out[c];
+            for (int c = 0; c < nc; c++) in[c] = src[(size_t)ta.field[c] * npts + p2];
+            tensor_transform<TT, false>(t2, in, b);
+#pragma unroll
+            for (int c = 0; c < nc; c++) {
+                dst[(size_t)(ta.dof0 + c) * npts + pe] = a[c] + b[c];
+                dst[(size_t)(ta.dof0 + c) * npts + po] = a[c] - b[c];
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < nc; c++) dst[(size_t)(ta.dof0 + c) * npts + pe] = a[c];
+        }
+    } else {
+        double out[nc];
+        if (paired) {
+#pragma unroll
+            for (int c = 0; c < nc; c++) {
+                const double e = src[(size_t)(ta.dof0 + c) * npts + pe], o = src[(size_t)(ta.dof0 + c) * npts + po];
+                a[c] = e + o; b[c] = e - o;
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < nc; c++) a[c] = src[(size_t)(ta.dof0 + c) * npts + pe];
+        }
+        tensor_transform<TT, true>(t1, a, out);
+#pragma unroll
+        for (int c = 0; c < nc; c++) dst[(size_t)ta.field[c] * npts + p1] = out[c];
+        if (paired) {
+            const Trig t2 = {st, ct, sin_p[j2], cos_p[j2]};
+            tensor_transform<TT, true>(t2, b, out);
+#pragma unroll
+            for (int c = 0; c < nc; c++) dst[(size_t)ta.field[c] * npts + p2] = out[c];
+        }
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// theta step (eq. 62).  coef[dof][mc][i][k], mc = 0: a_0; 2m-1: a_m; 2m: b_m.
+// theta step (eq. 62).  coef[dof][mc][i][k], mc = m: a_m (m = 0..L); mc = L+m: b_m (m = 1..L).
 // One CTA per (component, m); warp = column tile of 4 radii x {v = 0, 1} (columns interleaved
 // col = 2k + v so that a lane's two accumulator columns are the (v=0, v=1) pair of one radius).
 //   real component (n = 0):      a~_m = F^0_m a_m,  b~_m = F^0_m b_m
@@ -256,7 +304,7 @@ k_theta(ThetaBatch comps, const double *__restrict__ F, int L, int Nt, int Nt8, 
     const size_t dofsz = (size_t)MC4 * vec;
     const size_t fsz = (size_t)Nt8 * Nt4;
     if (4 * warp >= Nr) return;
-    const int mca = (m == 0) ? 0 : 2 * m - 1, mcb = 2 * m;
+    const int mca = m, mcb = L + m;                            // rows a_0..a_L, b_1..b_L
     const int kB = 4 * warp + (g >> 1), vB = g & 1;           // B-fragment column of this lane
     const bool kBok = kB < Nr;
     double acc1[MT][2], acc2[MT][2];

@@ -1,5 +1,5 @@
 // theta step of the Yn filter (eq. 61-62; 374-376), shared-memory staged.
-//   coef[dof][mc][i][k]  (mc = 0: a_0; 2m-1: a_m; 2m: b_m)  ->  cout, same layout
+//   coef[dof][mc][i][k]  (mc = m: a_m, m = 0..L; mc = L+m: b_m, m = 1..L)  ->  cout, same layout
 // CTA = (component, m, block of 36 radii).  K (= latitude ii) is walked in chunks of 8 through a 4-stage
 // cp.async pipeline holding the F^n_m rows (and F^{-n}_m for complex components) and the raw coefficient
 // rows a_m, b_m (real) or a^r, b^r, a^i, b^i (complex) of the CTA's radii.
@@ -44,7 +44,7 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp % mgroups, ng = warp / mgroups;
     const size_t vec = (size_t)Nt * Nr, dofsz = (size_t)MC4 * vec, fsz = (size_t)Nt8 * Nt8;
-    const int mca = (m == 0) ? 0 : 2 * m - 1, mcb = 2 * m;
+    const int mca = m, mcb = L + m;                            // rows a_0..a_L, b_1..b_L
     const int stageA = NMAT * Nt8 * TH_PA, stageB = NARR * TH_KC * TH_PKB;
     double *As = sm, *Bs = sm + TH_STAGES * stageA;
     const int nrad = min(TH_RC, Nr - k0);

@@ -22,9 +22,12 @@ struct sp_shell {
     double *d_sy = nullptr;        // Fourier synthesis [J8][MC4], zero padded         (eq. 23)
     double *d_F = nullptr;         // F^n_m [7][L+1][Nt8][Nt4], zero padded            (eq. 62)
     // shared-memory-staged phi GEMM operands: rows padded to the warp tiling, K padded to 8, zero filled
-    double *d_fd3p = nullptr, *d_anp = nullptr, *d_syp = nullptr;
-    int fd3_MT = 0, fd3_mg = 0, fd3_Mpad = 0, an_MT = 0, an_mg = 0, an_Mpad = 0, sy_MT = 0, sy_mg = 0, sy_Mpad = 0;
-    int Np8 = 0, MCk8 = 0;        // K of d/dphi and analysis (Np) / synthesis (MC) rounded up to 8
+    double *d_fd3p = nullptr;
+    int fd3_MT = 0, fd3_mg = 0, fd3_Mpad = 0;
+    int Np8 = 0;                  // K of d/dphi (Np) rounded up to 8
+    // folded Fourier matrices (phi -> 2 pi - phi reflection, see k_pointwise): cosine / sine blocks of analysis and synthesis
+    struct PhiMat { double *d = nullptr; int M = 0, K = 0, K8 = 0, MT = 0, mg = 0, Mpad = 0; };
+    PhiMat m_ac, m_as, m_sc, m_ss;   // analysis cos [L+1][J/2+1], sin [L][J/2-1]; synthesis cos [J/2+1][L+1], sin [J/2-1][L]
     double *d_inv_r = nullptr, *d_sin_t = nullptr, *d_cos_t = nullptr, *d_inv_sin_t = nullptr, *d_sin_p = nullptr,
            *d_cos_p = nullptr;     // Jacobian / triad factors                          (eq. 6, 51)
     // optional per-stage timing (sp_profile_enable): events recorded on the caller's stream

@@ -61,7 +61,7 @@ extern "C" sp_status sp_shell_create(int Nr, int Nt, int Np, double rin, double 
 }
 
 static void free_dev(sp_shell *s) {
-    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_fd3p, &s->d_anp, &s->d_syp, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
+    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_fd3p, &s->m_ac.d, &s->m_as.d, &s->m_sc.d, &s->m_ss.d, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
                     &s->d_inv_sin_t, &s->d_sin_p, &s->d_cos_p};
     for (auto q : p) {
         if (*q) cudaFree(*q);
@@ -125,22 +125,28 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
                     f[((size_t)q * s->Nt8 + i) * s->Nt8 + j] = H.F[((size_t)q * Nt + i) * Nt + j];
         if ((st = upload(&s->d_F, f.data(), f.size())) != SP_OK) return st;
     }
-    {   // padded operands of k_phi_gemm
-        PhiTiling t1 = phi_tiling(Np), t2 = phi_tiling(s->MC), t3 = phi_tiling(Np);
+    {   // padded operands of k_phi_gemm: FD_{Np}, and the folded Fourier blocks (entries taken from H.an / H.sy)
+        PhiTiling t1 = phi_tiling(Np);
         s->fd3_MT = t1.MT; s->fd3_mg = t1.mgroups; s->fd3_Mpad = t1.Mpad;
-        s->an_MT = t2.MT; s->an_mg = t2.mgroups; s->an_Mpad = t2.Mpad;
-        s->sy_MT = t3.MT; s->sy_mg = t3.mgroups; s->sy_Mpad = t3.Mpad;
-        s->Np8 = round_up(Np, 8); s->MCk8 = round_up(s->MC, 8);
-        std::vector<double> a((size_t)t1.Mpad * s->Np8, 0.0), b((size_t)t2.Mpad * s->Np8, 0.0), c((size_t)t3.Mpad * s->MCk8, 0.0);
+        s->Np8 = round_up(Np, 8);
+        std::vector<double> a((size_t)t1.Mpad * s->Np8, 0.0);
         for (int i = 0; i < Np; i++)
             for (int j = 0; j < Np; j++) a[(size_t)i * s->Np8 + j] = H.g3[((i - j) % Np + Np) % Np];
-        for (int m = 0; m < s->MC; m++)
-            for (int j = 0; j < Np; j++) b[(size_t)m * s->Np8 + j] = H.an[(size_t)m * Np + j];
-        for (int j = 0; j < Np; j++)
-            for (int m = 0; m < s->MC; m++) c[(size_t)j * s->MCk8 + m] = H.sy[(size_t)j * s->MC + m];
         if ((st = upload(&s->d_fd3p, a.data(), a.size())) != SP_OK) return st;
-        if ((st = upload(&s->d_anp, b.data(), b.size())) != SP_OK) return st;
-        if ((st = upload(&s->d_syp, c.data(), c.size())) != SP_OK) return st;
+        const int MC = s->MC, h = Nt;                 // h = J/2
+        auto mk = [&](sp_shell::PhiMat &pm, int M, int K, auto entry) -> sp_status {
+            PhiTiling tl = phi_tiling(M > 0 ? M : 1);
+            pm.M = M; pm.K = K; pm.K8 = round_up(K > 0 ? K : 1, 8); pm.MT = tl.MT; pm.mg = tl.mgroups; pm.Mpad = tl.Mpad;
+            std::vector<double> v((size_t)pm.Mpad * pm.K8, 0.0);
+            for (int r = 0; r < M; r++)
+                for (int c = 0; c < K; c++) v[(size_t)r * pm.K8 + c] = entry(r, c);
+            return upload(&pm.d, v.data(), v.size());
+        };
+        // rows of H.an: 0 = a_0, 2m-1 = a_m, 2m = b_m; columns of H.sy likewise
+        if ((st = mk(s->m_ac, L + 1, h + 1, [&](int m, int j) { return H.an[(size_t)(m == 0 ? 0 : 2 * m - 1) * Np + j]; })) != SP_OK) return st;
+        if ((st = mk(s->m_as, L, h - 1, [&](int r, int c) { return H.an[(size_t)(2 * (r + 1)) * Np + (c + 1)]; })) != SP_OK) return st;
+        if ((st = mk(s->m_sc, h + 1, L + 1, [&](int j, int m) { return H.sy[(size_t)j * MC + (m == 0 ? 0 : 2 * m - 1)]; })) != SP_OK) return st;
+        if ((st = mk(s->m_ss, h - 1, L, [&](int r, int c) { return H.sy[(size_t)(r + 1) * MC + 2 * (c + 1)]; })) != SP_OK) return st;
     }
     if ((st = upload(&s->d_inv_r, H.inv_r.data(), Nr)) != SP_OK) return st;
     if ((st = upload(&s->d_sin_t, H.sin_t.data(), Nt)) != SP_OK) return st;
@@ -376,7 +382,7 @@ static void tt_components(int tt, int dof0, std::vector<ThetaComp> &out) {
 template <bool INV>
 static void launch_pointwise(int tt, const TensorArgs &ta, const sp_shell *s, const double *src, double *dst, cudaStream_t st) {
     const int T = 128;
-    const unsigned nb = (unsigned)((s->npts + T - 1) / T);
+    const unsigned nb = (unsigned)(((size_t)s->Nr * s->Nt * (s->Nt + 1) + T - 1) / T);
 #define SP_PW(TTV)                                                                                                        \
     case TTV:                                                                                                             \
         k_pointwise<TTV, INV><<<nb, T, 0, st>>>(ta, s->Nr, s->Nt, s->npts, s->d_sin_t, s->d_cos_t, s->d_sin_p, s->d_cos_p, \
@@ -431,14 +437,21 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     sp_mark(s, st, 3);
     for (int t = 0; t < ntens; t++) launch_pointwise<false>(types[t], targs[t], s, u, dofs, st);
     sp_mark(s, st, 4);
-    g_sp_launches += 2 * ntens + 2;
-    // ---- F2: phi analysis (eq. 33)
-    PhiTiling tla = {s->an_MT, s->an_mg, s->an_Mpad}, tls = {s->sy_MT, s->sy_mg, s->sy_Mpad};
-    sp_status e = launch_phi_gemm(s->d_anp, s->Np8, s->MC, tla, Np, dofs, (long)vec, (long)npts, coef1, (long)vec, (long)(s->MC4 * vec),
-                                  (int)vec, ndof, st);
-    if (e == SP_ERR_UNSUPPORTED)
-        e = launch_gemm_cols<false>(s->d_an, Np, s->MC, Np, dofs, (long)vec, (long)npts, coef1, (long)vec, (long)(s->MC4 * vec),
-                                    (int)vec, ndof, st);
+    g_sp_launches += 2 * ntens;
+    // ---- F2: phi analysis (eq. 33) on the folded rows: cosine block -> a_0..a_L, sine block -> b_1..b_L
+    auto phi = [&](const sp_shell::PhiMat &pm, const double *B, long sBb, double *C, long sCb) -> sp_status {
+        if (pm.M <= 0 || pm.K <= 0) return SP_OK;
+        PhiTiling tl = {pm.MT, pm.mg, pm.Mpad};
+        sp_status e = launch_phi_gemm(pm.d, pm.K8, pm.M, tl, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, ndof, st);
+        if (e == SP_ERR_UNSUPPORTED)      // odd strides: generic global-memory kernel (same padded matrix)
+            e = launch_gemm_cols<false>(pm.d, pm.K8, pm.M, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, ndof, st);
+        g_sp_launches += 1;
+        return e;
+    };
+    const long cst = (long)(s->MC4 * vec);
+    sp_status e = phi(s->m_ac, dofs, (long)npts, coef1, cst);
+    if (e != SP_OK) return e;
+    e = phi(s->m_as, dofs + (size_t)(Nt + 1) * vec, (long)npts, coef1 + (size_t)(s->L + 1) * vec, cst);
     if (e != SP_OK) return e;
     sp_mark(s, st, 5);
     // ---- F3: per-(n,m) theta matrices (eq. 62)
@@ -487,13 +500,14 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
     }
     sp_mark(s, st, 6);
-    // ---- F4: phi synthesis (eq. 31)
-    e = launch_phi_gemm(s->d_syp, s->MCk8, Np, tls, s->MC, coef2, (long)vec, (long)(s->MC4 * vec), dofs, (long)vec, (long)npts, (int)vec,
-                        ndof, st);
-    if (e == SP_ERR_UNSUPPORTED)
-        e = launch_gemm_cols<false>(s->d_sy, s->MC4, Np, s->MC, coef2, (long)vec, (long)(s->MC4 * vec), dofs, (long)vec, (long)npts,
-                                    (int)vec, ndof, st);
+    // ---- F4: phi synthesis (eq. 31) into the folded rows: e_j (cosine block), o_j (sine block)
+    e = phi(s->m_sc, coef2, cst, dofs, (long)npts);
     if (e != SP_OK) return e;
+    e = phi(s->m_ss, coef2 + (size_t)(s->L + 1) * vec, cst, dofs + (size_t)(Nt + 1) * vec, (long)npts);
+    if (e != SP_OK) return e;
+    if (s->m_ss.K <= 0 && Nt > 1)      // L = 0: no sine modes survive, the odd rows o_j are zero
+        SP_CUDA(cudaMemset2DAsync(dofs + (size_t)(Nt + 1) * vec, npts * sizeof(double), 0, (size_t)(Nt - 1) * vec * sizeof(double),
+                                  (size_t)ndof, st));
     sp_mark(s, st, 7);
     // ---- F5: recombination
     for (int t = 0; t < ntens; t++) launch_pointwise<true>(types[t], targs[t], s, dofs, out, st);
