@@ -1,6 +1,6 @@
 // theta step of the Yn filter (eq. 61-62; 374-376), shared-memory staged.
 //   coef[dof][mc][i][k]  (mc = m: a_m, m = 0..L; mc = L+m: b_m, m = 1..L)  ->  cout, same layout
-// CTA = (component, m, block of 36 radii).  K (= latitude ii) is walked in chunks of 8 through a 4-stage
+// CTA = (component, m, block of 36 radii).  K (= latitude ii) is walked in chunks of 16 through a 3-stage
 // cp.async pipeline holding the F^n_m rows (and F^{-n}_m for complex components) and the raw coefficient
 // rows a_m, b_m (real) or a^r, b^r, a^i, b^i (complex) of the CTA's radii.
 // Warp (mg, ng): MT latitude tiles x 3 column tiles; a column tile is 4 radii x {v = 0, 1} interleaved
@@ -18,9 +18,9 @@
 #define TH_NGC 3
 #define TH_RC (TH_NGC * TH_NT * 4)     // 36 radii per CTA
 #define TH_PKB 37
-#define TH_KC 8
-#define TH_STAGES 4
-#define TH_PA 12
+#define TH_KC 16
+#define TH_STAGES 3
+#define TH_PA 20
 
 __device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
     unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -52,13 +52,16 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     const double *srcR = coef + (size_t)cmp.dof * dofsz + k0;            // arr = 2*part + (0: a_m, 1: b_m)
     const double *F0 = F2 + ((size_t)(3 + cmp.n) * (L + 1) + m) * fsz;
     const long dF = CPLX ? -2L * cmp.n * (long)(L + 1) * (long)fsz : 0L;   // F^{-n}_m relative to F^n_m
-    const int nchunks = Nt8 / TH_KC;
+    const int nchunks = (Nt8 + TH_KC - 1) / TH_KC;
 
     auto load_chunk = [&](int kc, int st) {
         double *as = As + st * stageA;
-        for (int q = tid; q < NMAT * Nt8 * 4; q += blockDim.x) {
-            const int mat = q / (Nt8 * 4), r = (q >> 2) % Nt8, h = q & 3;
-            cp_async16(as + (mat * Nt8 + r) * TH_PA + 2 * h, F0 + mat * dF + (size_t)r * Nt8 + kc * TH_KC + 2 * h);
+        for (int q = tid; q < NMAT * Nt8 * (TH_KC / 2); q += blockDim.x) {
+            const int rr = q >> 3, h = q & 7;                       // TH_KC / 2 = 8 sixteen-byte pieces per row
+            const int mat = (rr >= Nt8) ? 1 : 0, r = rr - mat * Nt8;
+            double *dst = as + rr * TH_PA + 2 * h;
+            if (kc * TH_KC + 2 * h < Nt8) cp_async16(dst, F0 + mat * dF + (size_t)r * Nt8 + kc * TH_KC + 2 * h);
+            else { dst[0] = 0.0; dst[1] = 0.0; }
         }
         double *bs = Bs + st * stageB;
         for (int q = tid; q < NARR * TH_KC * TH_RC; q += blockDim.x) {
