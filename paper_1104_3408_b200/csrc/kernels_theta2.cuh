@@ -42,7 +42,7 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     const int m = blockIdx.x;
     const int k0 = blockIdx.z * TH_RC;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-    const int mg = warp % mgroups, ng = warp / mgroups;
+    const int mg = warp % mgroups, ng = warp / mgroups, nwarps = blockDim.x >> 5;
     const size_t vec = (size_t)Nt * Nr, dofsz = (size_t)MC4 * vec, fsz = (size_t)Nt8 * Nt8;
     const int mca = m, mcb = L + m;                            // rows a_0..a_L, b_1..b_L
     const int stageA = NMAT * Nt8 * TH_PA, stageB = NARR * TH_KC * TH_PKB;
@@ -63,14 +63,18 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
             if (kc * TH_KC + 2 * h < Nt8) cp_async16(dst, F0 + mat * dF + (size_t)r * Nt8 + kc * TH_KC + 2 * h);
             else { dst[0] = 0.0; dst[1] = 0.0; }
         }
+        // raw coefficient rows: one (array, latitude) row of 36 radii per warp iteration, lane = radius
         double *bs = Bs + st * stageB;
-        for (int q = tid; q < NARR * TH_KC * TH_RC; q += blockDim.x) {
-            const int arr = q / (TH_KC * TH_RC), r = (q / TH_RC) % TH_KC, k = q % TH_RC;
+        for (int row = warp; row < NARR * TH_KC; row += nwarps) {
+            const int arr = row / TH_KC, r = row % TH_KC;
             const int ii = kc * TH_KC + r;
-            double *dst = bs + (arr * TH_KC + r) * TH_PKB + k;
-            const bool live = ii < Nt && k < nrad && !(m == 0 && (arr & 1));       // b_0 does not exist
-            if (live) cp_async8(dst, srcR + (size_t)(arr >> 1) * dofsz + (size_t)((arr & 1) ? mcb : mca) * vec + (size_t)ii * Nr + k);
-            else *dst = 0.0;
+            const bool rowlive = ii < Nt && !(m == 0 && (arr & 1));                     // b_0 does not exist
+            const double *srow = srcR + (size_t)(arr >> 1) * dofsz + (size_t)((arr & 1) ? mcb : mca) * vec + (size_t)ii * Nr;
+            double *drow = bs + row * TH_PKB;
+            if (rowlive && lane < nrad) cp_async8(drow + lane, srow + lane); else drow[lane] = 0.0;
+            if (lane < TH_RC - 32) {
+                if (rowlive && lane + 32 < nrad) cp_async8(drow + 32 + lane, srow + 32 + lane); else drow[32 + lane] = 0.0;
+            }
         }
     };
 
