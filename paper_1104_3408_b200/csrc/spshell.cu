@@ -9,6 +9,7 @@
 #include <cstdint>
 
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 #include <cstdlib>
 #include <new>
@@ -214,14 +215,41 @@ sp_status sp_configure_kernels(sp_shell *s) {
     if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;       // (r,theta) plane pair must fit one SM's shared memory
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    const size_t sm2 = grad2_smem_bytes(s->Nt, s->Nt8, s->Nr8, s->PU, s->gradKT);
-    if (sm2 > 227 * 1024) return SP_ERR_UNSUPPORTED;
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<3, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<5, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    {   // persistent (r,theta) kernel: two configurations, planes double-buffered (NBUF = 2) or not
+        const int itiles = s->Nt8 / 8, ktiles = s->Nr8 / 8, KT = s->gradKT;
+        const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
+        s->grad_nwarps = (KT == 3) ? std::min(ntasks, 12) : std::min(ntasks, 6);
+        cudaDeviceProp prop;
+        SP_CUDA(cudaGetDeviceProperties(&prop, 0));
+        s->num_sms = prop.multiProcessorCount;
+        for (int nb = 1; nb <= 2; nb++) {
+            s->grad_smem[nb - 1] = grad2_smem_bytes(s->Nt, s->Nt8, s->Nr8, s->PU, KT, nb, s->grad_nwarps);
+            s->grad_ctas[nb - 1] = 0;
+        }
+        if (s->grad_smem[0] > 227 * 1024) return SP_ERR_UNSUPPORTED;
+#define SP_GR_ATTR(KT_, SPL_, NB_)                                                                                      \
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<KT_, SPL_, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,           \
+                                 (int)s->grad_smem[NB_ - 1]));                                                          \
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<KT_, SPL_, NB_>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        SP_GR_ATTR(3, true, 1) SP_GR_ATTR(5, true, 1) SP_GR_ATTR(3, false, 1) SP_GR_ATTR(5, false, 1)
+        if (s->grad_smem[1] <= 227 * 1024) { SP_GR_ATTR(3, true, 2) SP_GR_ATTR(5, true, 2) SP_GR_ATTR(3, false, 2) SP_GR_ATTR(5, false, 2) }
+#undef SP_GR_ATTR
+        // resident CTAs per SM of the persistent grid, asked from the occupancy calculator for the variant that will run
+        for (int nb = 1; nb <= 2; nb++) {
+            if (s->grad_smem[nb - 1] > 227 * 1024) continue;
+            int occ = 0;
+            const int thr = s->grad_nwarps * 32;
+            if (KT == 3) {
+                if (nb == 1) SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grad_rtheta2<3, true, 1>, thr, s->grad_smem[0]));
+                else SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grad_rtheta2<3, true, 2>, thr, s->grad_smem[1]));
+            } else {
+                if (nb == 1) SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grad_rtheta2<5, true, 1>, thr, s->grad_smem[0]));
+                else SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grad_rtheta2<5, true, 2>, thr, s->grad_smem[1]));
+            }
+            s->grad_ctas[nb - 1] = occ;
+        }
+        if (s->grad_ctas[0] <= 0) return SP_ERR_UNSUPPORTED;
+    }
     const int pg = (int)((size_t)PG_STAGES * ((size_t)4 * 6 * 8 * PG_PA + PG_KC * PG_PB) * sizeof(double));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
@@ -276,7 +304,7 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     p.cd = s->d_cd; p.g2 = s->d_g2;
     p.inv_r = s->d_inv_r; p.sin_t = s->d_sin_t; p.cos_t = s->d_cos_t; p.inv_sin_t = s->d_inv_sin_t;
     p.sin_p = s->d_sin_p; p.cos_p = s->d_cos_p;
-    p.u = u; p.dphi = nullptr; p.du = du; p.nf = nf;
+    p.u = u; p.dphi = nullptr; p.du = du; p.nf = nf; p.nitems = Nt * nf;
     const dim3 grid(Nt, nf);
     PhiTiling tl = {s->fd3_MT, s->fd3_mg, s->fd3_Mpad};
     g_sp_launches += 2;
@@ -287,9 +315,18 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     if (Nt % 4 == 0 && s->grad_split_ok && aligned) {
         const int KT = s->gradKT;
         const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
-        const size_t sm2 = grad2_smem_bytes(Nt, s->Nt8, s->Nr8, s->PU, KT);
-        if (KT == 3) k_grad_rtheta2<3, true><<<grid, (ntasks < 12 ? ntasks : 12) * 32, sm2, st>>>(p);
-        else k_grad_rtheta2<5, true><<<grid, (ntasks < 6 ? ntasks : 6) * 32, sm2, st>>>(p);
+#define SPLITV true
+        // double-buffered planes pay off once every persistent CTA gets >= 3 items; small launches keep more CTAs per SM
+        const int nthr = s->grad_nwarps * 32;
+        const int nb = (s->grad_ctas[1] > 0 && p.nitems >= 3 * s->num_sms * s->grad_ctas[1]) ? 2 : 1;
+        const int ncta = std::min(p.nitems, s->num_sms * s->grad_ctas[nb - 1]);
+        const size_t smb = s->grad_smem[nb - 1];
+#define SP_GR_LAUNCH2(KT_, NB_) k_grad_rtheta2<KT_, SPLITV, NB_><<<ncta, nthr, smb, st>>>(p)
+        if (KT == 3) { if (nb == 2) SP_GR_LAUNCH2(3, 2); else SP_GR_LAUNCH2(3, 1); }
+        else { if (nb == 2) SP_GR_LAUNCH2(5, 2); else SP_GR_LAUNCH2(5, 1); }
+#undef SP_GR_LAUNCH2
+        (void)ntasks;
+#undef SPLITV
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         sp_mark(s, st, 1);
         PhiGradEpi ge = {du + (size_t)nf * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
@@ -312,9 +349,18 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     if (Nt % 4 == 0) {
         const int KT = s->gradKT;
         const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
-        const size_t sm2 = grad2_smem_bytes(Nt, s->Nt8, s->Nr8, s->PU, KT);
-        if (KT == 3) k_grad_rtheta2<3, false><<<grid, (ntasks < 12 ? ntasks : 12) * 32, sm2, st>>>(p);
-        else k_grad_rtheta2<5, false><<<grid, (ntasks < 6 ? ntasks : 6) * 32, sm2, st>>>(p);
+#define SPLITV false
+        // double-buffered planes pay off once every persistent CTA gets >= 3 items; small launches keep more CTAs per SM
+        const int nthr = s->grad_nwarps * 32;
+        const int nb = (s->grad_ctas[1] > 0 && p.nitems >= 3 * s->num_sms * s->grad_ctas[1]) ? 2 : 1;
+        const int ncta = std::min(p.nitems, s->num_sms * s->grad_ctas[nb - 1]);
+        const size_t smb = s->grad_smem[nb - 1];
+#define SP_GR_LAUNCH2(KT_, NB_) k_grad_rtheta2<KT_, SPLITV, NB_><<<ncta, nthr, smb, st>>>(p)
+        if (KT == 3) { if (nb == 2) SP_GR_LAUNCH2(3, 2); else SP_GR_LAUNCH2(3, 1); }
+        else { if (nb == 2) SP_GR_LAUNCH2(5, 2); else SP_GR_LAUNCH2(5, 1); }
+#undef SP_GR_LAUNCH2
+        (void)ntasks;
+#undef SPLITV
     } else {   // Ntheta not a multiple of 4: generic kernel
         const int ntasks = 2 * itiles * ((ktiles + 4) / 5);
         k_grad_rtheta<5><<<grid, (ntasks < 16 ? ntasks : 16) * 32, grad_smem_bytes(s), st>>>(p);
