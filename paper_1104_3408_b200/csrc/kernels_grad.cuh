@@ -315,6 +315,159 @@ __global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_r
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// v3: as k_grad_rtheta2<.., SPLIT = true, ..> plus the REFLECTION FOLD of the theta derivative.  FD_{2Ntheta} is an
+// antisymmetric circulant and the double cover is [own plane ascending | antipodal plane descending], so with
+// E = (P_j + P_{j+Ntheta})/2, O = (P_j - P_{j+Ntheta})/2 (formed in shared memory)
+//     d_theta P_j = G+ E + G- O,   d_theta P_{j+Ntheta} = G+ E - G- O,   G+-[i][r] = g(i - r) +- g(i + r + 1),
+// two Ntheta x Ntheta products instead of two Ntheta x 2Ntheta ones: the same sums regrouped, half the DMMAs.  d/dr is
+// linear, so it is taken on E and O as well and the planes are unfolded in the lane-local epilogue.
+// Warp task = (latitude tile, group of KT radial tiles), four accumulator sets (theta/r x E/O).
+// ---------------------------------------------------------------------------------------------
+template <int KT, int NBUF>
+__global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_rtheta3(GradParams p) {
+    extern __shared__ double sm[];
+    const int Nr = p.Nr, Nt = p.Nt, Np = p.Np, PU = p.PU;
+    const int itiles = p.Nt8 >> 3, ipairs = (itiles + 1) >> 1, ktiles = p.Nr8 >> 3, kgroups = (ktiles + KT - 1) / KT;
+    const int NK8 = kgroups * KT * 8, n2 = 2 * Nt;
+    const int prow = p.Nt8 + ((itiles & 1) ? 8 : 0);           // rows of a plane buffer
+    const size_t planesz = (size_t)prow * PU;
+    double *CDs = sm, *g2d = CDs + (size_t)NK8 * PU;
+    double *tir = g2d + 2 * n2 + 8, *tst = tir + NK8, *tct = tst + p.Nt8 + 8, *tis = tct + p.Nt8 + 8;   // 1/r, sin, cos, 1/sin(theta)
+    double *Pbuf = tis + p.Nt8 + 8;                                                                     // NBUF x [P0, P1]
+    const size_t npts = (size_t)Nr * Nt * Np, plane = (size_t)Nr * Nt;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+
+    // planes of one item: one latitude row per warp iteration, 8-byte cp.async into the padded pitch
+    auto issue_planes = [&](int it, double *B0) {
+        const int mu_ = it / Nt, j_ = it - mu_ * Nt;
+        const double *u0 = p.u + mu_ * npts + (size_t)j_ * plane, *u1 = u0 + (size_t)Nt * plane;
+        double *B1 = B0 + planesz;
+        for (int i = warp; i < Nt; i += nwarps)
+            for (int k = lane; k < Nr; k += 32) {
+                cp_async8g(B0 + i * PU + k, u0 + (size_t)i * Nr + k);
+                cp_async8g(B1 + i * PU + k, u1 + (size_t)i * Nr + k);
+            }
+    };
+    // padding (columns >= Nr, rows >= Nt) of every buffer: zero, once
+    for (int bq = 0; bq < 2 * NBUF; bq++) {
+        double *B = Pbuf + bq * planesz;
+        for (int i = warp; i < prow; i += nwarps)
+            for (int k = lane; k < PU; k += 32)
+                if (!(i < Nt && k < Nr)) B[i * PU + k] = 0.0;
+    }
+    // CD^ rows (16-byte copies: the pitch PU is even), circulant table and Jacobian tables: all asynchronous
+    for (int q = threadIdx.x; q < NK8 * (PU / 2); q += blockDim.x) {
+        const int r = q / (PU / 2), h = q - r * (PU / 2);
+        if (r < p.Nr8) {
+            unsigned sa = (unsigned)__cvta_generic_to_shared(CDs + r * PU + 2 * h);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(p.cd + r * PU + 2 * h));
+        } else {
+            CDs[r * PU + 2 * h] = 0.0; CDs[r * PU + 2 * h + 1] = 0.0;
+        }
+    }
+    for (int q = threadIdx.x; q < 2 * n2 + 8; q += blockDim.x) cp_async8g(g2d + q, p.g2 + (q % n2));
+    for (int q = threadIdx.x; q < NK8; q += blockDim.x) {
+        if (q < Nr) cp_async8g(tir + q, p.inv_r + q); else tir[q] = 0.0;
+    }
+    for (int q = threadIdx.x; q < p.Nt8 + 8; q += blockDim.x) {
+        if (q < Nt) { cp_async8g(tst + q, p.sin_t + q); cp_async8g(tct + q, p.cos_t + q); cp_async8g(tis + q, p.inv_sin_t + q); }
+        else { tst[q] = 0.0; tct[q] = 0.0; tis[q] = 0.0; }
+    }
+    if ((int)blockIdx.x < p.nitems) issue_planes(blockIdx.x, Pbuf);
+    asm volatile("cp.async.commit_group;\n" ::);
+
+    const int g = lane >> 2, t = lane & 3;
+    const int ntasks = itiles * kgroups;
+  int nloc = 0;
+  for (int it = blockIdx.x; it < p.nitems; it += gridDim.x, nloc++) {
+    const int mu = it / Nt, j = it - mu * Nt;
+    double *P0 = Pbuf + (size_t)(NBUF == 2 ? (nloc & 1) : 0) * 2 * planesz, *P1 = P0 + planesz;
+    if (NBUF == 2) {
+        const int nxt = it + gridDim.x;
+        if (nxt < p.nitems) issue_planes(nxt, Pbuf + (size_t)((nloc + 1) & 1) * 2 * planesz);
+        asm volatile("cp.async.commit_group;\n" ::);
+        asm volatile("cp.async.wait_group 1;\n" ::);
+    } else {
+        asm volatile("cp.async.wait_group 0;\n" ::);
+    }
+    __syncthreads();
+    // fold: E = (P0 + P1)/2, O = (P0 - P1)/2 in place (valid region; the padding stays zero)
+    for (int i = warp; i < Nt; i += nwarps)
+        for (int k = lane; k < Nr; k += 32) {
+            const double x = P0[i * PU + k], y = P1[i * PU + k];
+            P0[i * PU + k] = 0.5 * (x + y); P1[i * PU + k] = 0.5 * (x - y);
+        }
+    __syncthreads();
+    for (int task = warp; task < ntasks; task += nwarps) {
+        const int it_ = task / kgroups, kg = task - it_ * kgroups;
+        const int kt0 = kg * KT;
+        const int ir0 = it_ * 8 + g;                              // the lane's latitude row
+        double tE[KT][2], tO[KT][2], rE[KT][2], rO[KT][2];
+#pragma unroll
+        for (int q = 0; q < KT; q++) tE[q][0] = tE[q][1] = tO[q][0] = tO[q][1] = rE[q][0] = rE[q][1] = rO[q][0] = rO[q][1] = 0.0;
+        // ---- d/dtheta on the folded planes: Gp/m[i][r] = g(i - r) +/- g(i + r + 1), K = Ntheta
+        {
+            const double *ga = g2d + (ir0 - t + n2), *gb = g2d + (ir0 + t + 1);
+            const double *bE = P0 + t * PU + kt0 * 8 + g, *bO = P1 + t * PU + kt0 * 8 + g;
+#pragma unroll 2
+            for (int ks = 0; ks < Nt / 4; ks++) {
+                const double x = ga[-4 * ks], y = gb[4 * ks];
+                const double ap = x + y, am = x - y;
+#pragma unroll
+                for (int q = 0; q < KT; q++) {
+                    dmma(tE[q][0], tE[q][1], ap, bE[(size_t)ks * 4 * PU + q * 8]);
+                    dmma(tO[q][0], tO[q][1], am, bO[(size_t)ks * 4 * PU + q * 8]);
+                }
+            }
+        }
+        // ---- d/dr on E and O: A = plane rows, B[kk][k'] = CD^[k'][kk]   (eq. 9, 13)
+        {
+            const double *aE = P0 + ir0 * PU + t, *aO = P1 + ir0 * PU + t;
+            const double *cdp = CDs + (kt0 * 8 + g) * PU + t;
+#pragma unroll 3
+            for (int ks = 0; ks < p.Nr4 / 4; ks++) {
+                const double a0 = aE[ks * 4], a1 = aO[ks * 4];
+#pragma unroll
+                for (int q = 0; q < KT; q++) {
+                    const double bf = cdp[q * 8 * PU + ks * 4];
+                    dmma(rE[q][0], rE[q][1], a0, bf);
+                    dmma(rO[q][0], rO[q][1], a1, bf);
+                }
+            }
+        }
+        // ---- unfold (plane j: E + O, plane j + Ntheta: E - O) and the phi-independent part of the chain rule (eq. 6)
+        if (ir0 < Nt) {
+            const double st = tst[ir0], ct = tct[ir0];
+            const size_t fs = (size_t)p.nf * npts;
+            const size_t b0 = (size_t)mu * npts + (size_t)j * plane + (size_t)ir0 * Nr, b1 = b0 + (size_t)Nt * plane;
+#pragma unroll
+            for (int q = 0; q < KT; q++) {
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    const int k = (kt0 + q) * 8 + 2 * t + e;
+                    if (k < Nr) {
+                        const double ir = tir[k];
+                        const double r0 = rE[q][e] + rO[q][e], r1 = rE[q][e] - rO[q][e];
+                        const double t0 = (tE[q][e] + tO[q][e]) * ir, t1 = (tE[q][e] - tO[q][e]) * ir;
+                        p.du[b0 + k] = st * r0 + ct * t0;
+                        p.du[2 * fs + b0 + k] = ct * r0 - st * t0;
+                        p.du[b1 + k] = st * r1 + ct * t1;
+                        p.du[2 * fs + b1 + k] = ct * r1 - st * t1;
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();                       // every warp is done with this item's planes
+    if (NBUF == 1) {
+        const int nxt = it + gridDim.x;
+        if (nxt < p.nitems) issue_planes(nxt, Pbuf);
+        asm volatile("cp.async.commit_group;\n" ::);
+    }
+  }
+}
+
 // shared memory of k_grad_rtheta2<KT>
 static inline size_t grad2_smem_bytes(int Nt, int Nt8, int Nr8, int PU, int KT, int nbuf, int nwarps) {
     const int ktiles = Nr8 / 8, NK8 = ((ktiles + KT - 1) / KT) * KT * 8, itiles = Nt8 / 8;

@@ -10,7 +10,8 @@ struct sp_shell {
     double rin, rout;
     int Nr8, Nr4, Nt8, Nt4, MC, MC4, MC8, J8, PU;
     bool grad_split_ok = false;   // the split gradient (r-theta kernel first, d/dphi GEMM with fused chain rule) is usable
-    int grad_nwarps = 6, num_sms = 148;
+    int grad_nwarps = 6, grad3_nwarps = 6, num_sms = 148;
+    int grad3_ctas[2] = {0, 0};      // same for the folded kernel k_grad_rtheta3
     int grad_ctas[2] = {1, 0};       // resident CTAs per SM with NBUF = 1 / 2 (0: does not fit)
     size_t grad_smem[2] = {0, 0};
     int gradKT;                   // radial tiles per warp task of k_grad_rtheta2 (3 or 5)

@@ -249,6 +249,26 @@ sp_status sp_configure_kernels(sp_shell *s) {
             s->grad_ctas[nb - 1] = occ;
         }
         if (s->grad_ctas[0] <= 0) return SP_ERR_UNSUPPORTED;
+        // folded variant (k_grad_rtheta3): warp task = (latitude tile, radial group)
+        {
+            const int nt3 = itiles * ((ktiles + KT - 1) / KT);
+            s->grad3_nwarps = (KT == 3) ? std::min(nt3, 12) : std::min(nt3, 6);
+            const int thr = s->grad3_nwarps * 32;
+            for (int nb = 1; nb <= 2; nb++) {
+                s->grad3_ctas[nb - 1] = 0;
+                if (s->grad_smem[nb - 1] > 227 * 1024) continue;
+                int occ = 0;
+                const int smb = (int)s->grad_smem[nb - 1];
+#define SP_G3(KT_, NB_)                                                                                             \
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, smb));      \
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));   \
+    SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grad_rtheta3<KT_, NB_>, thr, smb));
+                if (KT == 3) { if (nb == 1) { SP_G3(3, 1) } else { SP_G3(3, 2) } }
+                else { if (nb == 1) { SP_G3(5, 1) } else { SP_G3(5, 2) } }
+#undef SP_G3
+                s->grad3_ctas[nb - 1] = occ;
+            }
+        }
     }
     const int pg = (int)((size_t)PG_STAGES * ((size_t)4 * 6 * 8 * PG_PA + PG_KC * PG_PB) * sizeof(double));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
@@ -315,6 +335,15 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     if (Nt % 4 == 0 && s->grad_split_ok && aligned) {
         const int KT = s->gradKT;
         const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
+        if (s->grad3_ctas[0] > 0) {      // folded theta derivative (k_grad_rtheta3)
+            const int nthr = s->grad3_nwarps * 32;
+            const int nb = (s->grad3_ctas[1] > 0 && p.nitems >= 3 * s->num_sms * s->grad3_ctas[1]) ? 2 : 1;
+            const int ncta = std::min(p.nitems, s->num_sms * s->grad3_ctas[nb - 1]);
+            const size_t smb = s->grad_smem[nb - 1];
+            if (KT == 3) { if (nb == 2) k_grad_rtheta3<3, 2><<<ncta, nthr, smb, st>>>(p); else k_grad_rtheta3<3, 1><<<ncta, nthr, smb, st>>>(p); }
+            else { if (nb == 2) k_grad_rtheta3<5, 2><<<ncta, nthr, smb, st>>>(p); else k_grad_rtheta3<5, 1><<<ncta, nthr, smb, st>>>(p); }
+            (void)ntasks;
+        } else {
 #define SPLITV true
         // double-buffered planes pay off once every persistent CTA gets >= 3 items; small launches keep more CTAs per SM
         const int nthr = s->grad_nwarps * 32;
@@ -327,6 +356,7 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
 #undef SP_GR_LAUNCH2
         (void)ntasks;
 #undef SPLITV
+        }
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         sp_mark(s, st, 1);
         PhiGradEpi ge = {du + (size_t)nf * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
