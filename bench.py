@@ -30,8 +30,8 @@ L2_BYTES = 126e6
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); default 3 = GHG-50 at 33x48x96")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs")
@@ -100,7 +100,7 @@ class ClockSampler:
 # CPU oracle leg (cpu_baseline and --impl reference): the oracle as it stands, on a bounded sample
 # ---------------------------------------------------------------------------------------------------
 ORACLE_SAMPLE = {   # config -> (fields differentiated, radii filtered) of the FIRST tensor of the state
-    1: (1, 9), 2: (10, 17), 3: (4, 4), 4: (1, 1), 5: (1, 2),
+    1: (1, 9), 2: (10, 17), 3: (2, 2), 4: (1, 1), 5: (1, 2),
 }
 
 
@@ -246,27 +246,53 @@ class GpuWorkload:
         return {k: statistics.median(r[k] for r in rows) for k in rows[0]}
 
     def e2e(self, steps):
-        """Same metric through the public API with HOST buffers: pinned host state -> device, gradient +
-        filter, results back to pinned host memory; copies inside the timed region."""
+        """Same metric through the public API with HOST buffers: every step copies its state from pinned host
+        memory to the device, runs gradient + filter, and copies the gradient and the filtered state back to
+        pinned host memory; all of it inside the timed region.  Copies and kernels of neighbouring steps overlap
+        on three streams (H2D, compute, D2H) with double-buffered device arrays -- PCIe is full duplex."""
         torch = self.torch
         hu = torch.from_numpy(self.u_host).pin_memory()
         hdu = torch.empty(self.du.shape, dtype=torch.float64).pin_memory()
         hfu = torch.empty(self.fu.shape, dtype=torch.float64).pin_memory()
-        ud = self.u[0]
+        s_in, s_c, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+        ud = [self.u[0], self.u[1 % self.nsets]]
+        du = [self.du, torch.empty_like(self.du)]
+        fu = [self.fu, torch.empty_like(self.fu)]
+        ev_in = [torch.cuda.Event() for _ in range(2)]
+        ev_c = [torch.cuda.Event() for _ in range(2)]
+        ev_out = [torch.cuda.Event() for _ in range(2)]
 
-        def one():
-            ud.copy_(hu, non_blocking=True)
-            self.sh.cartesian_gradient(ud, out=self.du, workspace=self.ws_g)
-            self.sh.tensor_filter(ud, self.cfg["tensors"], out=self.fu, workspace=self.ws_f, descs=self.descs)
-            hdu.copy_(self.du, non_blocking=True)
-            hfu.copy_(self.fu, non_blocking=True)
+        def one(n):
+            b = n & 1
+            with torch.cuda.stream(s_in):
+                s_in.wait_event(ev_c[b])              # compute of step n-2 has finished reading ud[b]
+                ud[b].copy_(hu, non_blocking=True)
+                ev_in[b].record(s_in)
+            with torch.cuda.stream(s_c):
+                s_c.wait_event(ev_in[b])
+                s_c.wait_event(ev_out[b])             # D2H of step n-2 has drained du[b], fu[b]
+                self.sh.cartesian_gradient(ud[b], out=du[b], workspace=self.ws_g, stream=s_c)
+                self.sh.tensor_filter(ud[b], self.cfg["tensors"], out=fu[b], workspace=self.ws_f, descs=self.descs, stream=s_c)
+                ev_c[b].record(s_c)
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(ev_c[b])
+                hdu.copy_(du[b], non_blocking=True)
+                hfu.copy_(fu[b], non_blocking=True)
+                ev_out[b].record(s_out)
 
-        one()
+        torch.cuda.synchronize()
+        for n in range(2):
+            one(n)
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        for _ in range(steps):
-            one()
+        for s_ in (s_in, s_c, s_out):
+            s_.wait_event(e0)
+        for n in range(steps):
+            one(n)
+        cur = torch.cuda.current_stream()
+        for s_ in (s_in, s_c, s_out):
+            ev = torch.cuda.Event(); ev.record(s_); cur.wait_event(ev)
         e1.record()
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / steps
@@ -332,7 +358,7 @@ def run_ours(args):
     value = units_all / (ms_all * 1e-3)
 
     # end to end with host buffers (every rank, max over ranks)
-    e2e_ms, h2d, d2h = wl.e2e(max(3, min(args.steps, 10)))
+    e2e_ms, h2d, d2h = wl.e2e(max(4, min(args.steps, 20)))
     e2e_ms_all, e2e_units = aggregate_over_ranks(e2e_ms, wl.units, dist if world > 1 else None)
     stages = wl.stage_times()
     if rank != 0:
@@ -371,7 +397,7 @@ def run_ours(args):
             torch.cuda.empty_cache()
             c2 = synth.config(cid)
             w2 = GpuWorkload(c2)
-            k2 = 10 if cid != 2 else 50
+            k2 = {2: 200, 4: 20, 5: 100}[cid]
             m2 = w2.time_steps(k2, 3)
             st2 = w2.stage_times()
             r2, t2 = roofline_for(c2, st2, w2.units, peak_tf, hbm_gbs, hbm_src)
