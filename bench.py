@@ -68,6 +68,27 @@ class ClockSampler:
         self.t = threading.Thread(target=self._run, daemon=True)
 
     def _run(self):
+        try:                                   # NVML in-process: a sample every few ms
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            mx = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
+            R = pynvml
+            bits = [("hw_slowdown", R.nvmlClocksEventReasonHwSlowdown), ("hw_thermal_slowdown", R.nvmlClocksEventReasonHwThermalSlowdown),
+                    ("sw_thermal_slowdown", R.nvmlClocksEventReasonSwThermalSlowdown), ("sw_power_cap", R.nvmlClocksEventReasonSwPowerCap)]
+            while not self.stop_flag:
+                sm = pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)
+                try:
+                    rs = pynvml.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    rs = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                pw = pynvml.nvmlDeviceGetPowerUsage(h) / 1e3
+                row = [str(sm), str(mx), str(pw)] + ["Active" if (rs & bit) else "Not Active" for _, bit in bits]
+                self.rows.append(row)
+                time.sleep(0.003)
+            return
+        except Exception:
+            pass
         while not self.stop_flag:
             try:
                 out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
