@@ -1,9 +1,9 @@
 // phi-direction contraction, shared-memory staged (the hot GEMM: d/dphi, phi analysis, phi synthesis).
 //     C[b][m][c] = sum_k A[m][k] * B[b][k][c],   B[b][k][c] = B + b*sBb + k*sBk + c  (columns contiguous)
 // (eq. 17-19 without the transposes; 254-259 eq. 33; 243-246 eq. 31.)
-// CTA tile = ALL rows of A x 64 columns; K walked in chunks of 8 through a 4-stage cp.async pipeline:
-//   As[stage][Mpad][12]  (pitch 12 doubles: fragment reads hit 16 distinct 8-byte banks)
-//   Bs[stage][8][68]     (pitch 68 = 4 mod 16: likewise)
+// CTA tile = ALL rows of A x 64 columns; K walked in chunks of 16 through a 3-stage cp.async pipeline:
+//   As[stage][Mpad][20]  (pitch 20 doubles: fragment reads hit 16 distinct 8-byte banks)
+//   Bs[stage][16][68]    (pitch 68 = 4 mod 16: likewise)
 // Warp (mg, ng): MT m-tiles x 2 n-tiles of 8x8, DMMA.8x8x4.  Requires even strides / ncols and 16-byte
 // aligned bases (checked by the launcher; otherwise the generic kernel of kernels_gemm.cuh is used).
 #pragma once
@@ -12,9 +12,9 @@
 #include <cstdint>
 
 #define PG_NCOL 64
-#define PG_KC 8
-#define PG_STAGES 4
-#define PG_PA 12
+#define PG_KC 16
+#define PG_STAGES 3
+#define PG_PA 20
 #define PG_PB 68
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
@@ -40,29 +40,31 @@ __global__ void __launch_bounds__(512)
 k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const double *__restrict__ B, long sBk, long sBb,
            double *__restrict__ C, long sCm, long sCb, int ncols, PhiGradEpi ge) {
     extern __shared__ __align__(16) double sm[];
-    const int stageA = Mpad * PG_PA, stageB = PG_KC * PG_PB;
-    double *As = sm, *Bs = sm + PG_STAGES * stageA;
-    double *Ws = Bs + PG_STAGES * stageB;
+    // plain products: K chunks of 16, 3 stages; gradient variant (which also holds the W tile): chunks of 8, 4 stages
+    constexpr int KC = EPI_GRAD ? 8 : 16, STG = EPI_GRAD ? 4 : 3, PA = KC + 4;
+    const int stageA = Mpad * PA, stageB = KC * PG_PB;
+    double *As = sm, *Bs = sm + STG * stageA;
+    double *Ws = Bs + STG * stageB;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp >> 2, ng = warp & 3;
     const int c0 = blockIdx.x * PG_NCOL;
     const double *Bb = B + (long)blockIdx.y * sBb + c0;
     double *Cb = C + (long)blockIdx.y * sCb + c0;
-    const int nchunks = (K + PG_KC - 1) / PG_KC;
+    const int nchunks = (K + KC - 1) / KC;
     const int colsleft = ncols - c0;                    // > 0, even
 
     auto load_chunk = [&](int kc, int st) {
         // A chunk: Mpad rows x 8 doubles (4 x 16 B per row); rows and K are zero padded in global memory
         double *as = As + st * stageA;
-        for (int q = tid; q < Mpad * 4; q += blockDim.x) {
-            const int r = q >> 2, h = q & 3;
-            cp_async16(as + r * PG_PA + 2 * h, A + (long)r * lda + kc * PG_KC + 2 * h);
+        for (int q = tid; q < Mpad * (KC / 2); q += blockDim.x) {
+            const int r = q / (KC / 2), h = q % (KC / 2);
+            cp_async16(as + r * PA + 2 * h, A + (long)r * lda + kc * KC + 2 * h);
         }
         // B chunk: 8 rows x 64 columns (32 x 16 B per row); rows >= K and columns >= ncols are zero-filled
         double *bs = Bs + st * stageB;
-        for (int q = tid; q < PG_KC * (PG_NCOL / 2); q += blockDim.x) {
+        for (int q = tid; q < KC * (PG_NCOL / 2); q += blockDim.x) {
             const int r = q >> 5, h = q & 31;
-            const int k = kc * PG_KC + r;
+            const int k = kc * KC + r;
             double *dst = bs + r * PG_PB + 2 * h;
             if (k < K && 2 * h < colsleft) cp_async16(dst, Bb + (long)k * sBk + 2 * h);
             else { dst[0] = 0.0; dst[1] = 0.0; }
@@ -83,22 +85,23 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
         cp_async_commit();
     }
 #pragma unroll
-    for (int s = 0; s < PG_STAGES - 1; s++) {
+    for (int s = 0; s < STG - 1; s++) {
         if (s < nchunks) load_chunk(s, s);
         cp_async_commit();
     }
     for (int kc = 0; kc < nchunks; kc++) {
-        cp_async_wait<PG_STAGES - 2>();
+        cp_async_wait<STG - 2>();
         __syncthreads();
-        if (kc + PG_STAGES - 1 < nchunks) load_chunk(kc + PG_STAGES - 1, (kc + PG_STAGES - 1) % PG_STAGES);
+        if (kc + STG - 1 < nchunks) load_chunk(kc + STG - 1, (kc + STG - 1) % STG);
         cp_async_commit();
-        const double *as = As + (kc % PG_STAGES) * stageA + (mg * MT * 8 + g) * PG_PA + t;
-        const double *bs = Bs + (kc % PG_STAGES) * stageB + t * PG_PB + ng * 16 + g;
-#pragma unroll
-        for (int ks = 0; ks < PG_KC / 4; ks++) {
+        const double *as = As + (kc % STG) * stageA + (mg * MT * 8 + g) * PA + t;
+        const double *bs = Bs + (kc % STG) * stageB + t * PG_PB + ng * 16 + g;
+        const int nks = min(KC / 4, (K - kc * KC + 3) >> 2);      // the last chunk may be short
+#pragma unroll 4
+        for (int ks = 0; ks < nks; ks++) {
             double af[MT], bf[2];
 #pragma unroll
-            for (int a = 0; a < MT; a++) af[a] = as[a * 8 * PG_PA + ks * 4];
+            for (int a = 0; a < MT; a++) af[a] = as[a * 8 * PA + ks * 4];
             bf[0] = bs[ks * 4 * PG_PB];
             bf[1] = bs[ks * 4 * PG_PB + 8];
 #pragma unroll
@@ -166,7 +169,8 @@ static inline PhiTiling phi_tiling(int M) {
     return best;
 }
 static inline size_t phi_smem_bytes(const PhiTiling &tl, int Mgrad = 0) {
-    return ((size_t)PG_STAGES * ((size_t)tl.Mpad * PG_PA + PG_KC * PG_PB) + (size_t)Mgrad * PG_PW) * sizeof(double);
+    const int KC = Mgrad ? 8 : 16, STG = Mgrad ? 4 : 3, PA = KC + 4;
+    return ((size_t)STG * ((size_t)tl.Mpad * PA + KC * PG_PB) + (size_t)Mgrad * PG_PW) * sizeof(double);
 }
 
 // returns SP_ERR_UNSUPPORTED when the fast-path preconditions do not hold (caller falls back)

@@ -129,7 +129,7 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
     {   // padded operands of k_phi_gemm: FD_{Np}, and the folded Fourier blocks (entries taken from H.an / H.sy)
         PhiTiling t1 = phi_tiling(Np);
         s->fd3_MT = t1.MT; s->fd3_mg = t1.mgroups; s->fd3_Mpad = t1.Mpad;
-        s->Np8 = round_up(Np, 8);
+        s->Np8 = round_up(Np, PG_KC);
         std::vector<double> a((size_t)t1.Mpad * s->Np8, 0.0);
         for (int i = 0; i < Np; i++)
             for (int j = 0; j < Np; j++) a[(size_t)i * s->Np8 + j] = H.g3[((i - j) % Np + Np) % Np];
@@ -137,7 +137,7 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
         const int MC = s->MC, h = Nt;                 // h = J/2
         auto mk = [&](sp_shell::PhiMat &pm, int M, int K, auto entry) -> sp_status {
             PhiTiling tl = phi_tiling(M > 0 ? M : 1);
-            pm.M = M; pm.K = K; pm.K8 = round_up(K > 0 ? K : 1, 8); pm.MT = tl.MT; pm.mg = tl.mgroups; pm.Mpad = tl.Mpad;
+            pm.M = M; pm.K = K; pm.K8 = round_up(K > 0 ? K : 1, PG_KC); pm.MT = tl.MT; pm.mg = tl.mgroups; pm.Mpad = tl.Mpad;
             std::vector<double> v((size_t)pm.Mpad * pm.K8, 0.0);
             for (int r = 0; r < M; r++)
                 for (int c = 0; c < K; c++) v[(size_t)r * pm.K8 + c] = entry(r, c);
@@ -270,7 +270,8 @@ sp_status sp_configure_kernels(sp_shell *s) {
             }
         }
     }
-    const int pg = (int)((size_t)PG_STAGES * ((size_t)4 * 6 * 8 * PG_PA + PG_KC * PG_PB) * sizeof(double));
+    PhiTiling tmax = {6, 4, 4 * 6 * 8};
+    const int pg = (int)phi_smem_bytes(tmax);
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
