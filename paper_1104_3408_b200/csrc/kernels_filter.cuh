@@ -214,11 +214,17 @@ __device__ __forceinline__ void tensor_transform(const Trig &q, const double *in
 // Folded dof arrays [dof][row][i][k]: rows 0..J/2 hold f_0, E_1..E_{J/2-1}, f_{J/2}; rows J/2+j hold O_j.
 // One thread owns the grid points (k, i, j) and (k, i, J-j), j = 0..J/2.
 //   INV = false: state fields -> folded dofs;   INV = true: folded dofs -> state fields.
+// tensors of the SAME index structure share one launch: blockIdx.y selects the tensor
+#define SP_PW_GROUP 4
+struct TensorArgsGroup { TensorArgs t[SP_PW_GROUP]; };
+
 template <int TT, bool INV>
 __global__ void __launch_bounds__(128)
-k_pointwise(TensorArgs ta, int Nr, int Nt, size_t npts, const double *__restrict__ sin_t, const double *__restrict__ cos_t,
-            const double *__restrict__ sin_p, const double *__restrict__ cos_p, const double *src, double *dst) {
+k_pointwise(const __grid_constant__ TensorArgsGroup tg, int Nr, int Nt, size_t npts, const double *__restrict__ sin_t,
+            const double *__restrict__ cos_t, const double *__restrict__ sin_p, const double *__restrict__ cos_p, const double *src,
+            double *dst) {
     constexpr int nc = TTInfo<TT>::nc;
+    const TensorArgs &ta = tg.t[blockIdx.y];
     const size_t plane = (size_t)Nr * Nt;
     const size_t q0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;       // (k, i, j) with j in [0, J/2]
     if (q0 >= plane * (size_t)(Nt + 1)) return;

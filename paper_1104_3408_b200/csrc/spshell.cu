@@ -457,19 +457,30 @@ static void tt_components(int tt, int dof0, std::vector<ThetaComp> &out) {
 }
 
 template <bool INV>
-static void launch_pointwise(int tt, const TensorArgs &ta, const sp_shell *s, const double *src, double *dst, cudaStream_t st) {
+static void launch_pointwise(const std::vector<int> &types, const std::vector<TensorArgs> &targs, const sp_shell *s, const double *src,
+                             double *dst, cudaStream_t st) {
     const int T = 128;
     const unsigned nb = (unsigned)(((size_t)s->Nr * s->Nt * (s->Nt + 1) + T - 1) / T);
+    std::vector<char> done(types.size(), 0);
+    for (size_t t0 = 0; t0 < types.size(); t0++) {
+        if (done[t0]) continue;
+        TensorArgsGroup tg;                      // this tensor and the following ones of the same index structure
+        int n = 0;
+        for (size_t t1 = t0; t1 < types.size() && n < SP_PW_GROUP; t1++)
+            if (!done[t1] && types[t1] == types[t0]) { tg.t[n++] = targs[t1]; done[t1] = 1; }
+        const dim3 grid(nb, n);
 #define SP_PW(TTV)                                                                                                        \
     case TTV:                                                                                                             \
-        k_pointwise<TTV, INV><<<nb, T, 0, st>>>(ta, s->Nr, s->Nt, s->npts, s->d_sin_t, s->d_cos_t, s->d_sin_p, s->d_cos_p, \
-                                                src, dst);                                                                \
+        k_pointwise<TTV, INV><<<grid, T, 0, st>>>(tg, s->Nr, s->Nt, s->npts, s->d_sin_t, s->d_cos_t, s->d_sin_p, s->d_cos_p, \
+                                                  src, dst);                                                              \
         break;
-    switch (tt) {
-        SP_PW(TT_SCALAR) SP_PW(TT_VEC3) SP_PW(TT_VEC4) SP_PW(TT_SYM3) SP_PW(TT_SYM4) SP_PW(TT_R3_3_3) SP_PW(TT_R3_3_4)
-        SP_PW(TT_R3_4_3) SP_PW(TT_R3_4_4)
-    }
+        switch (types[t0]) {
+            SP_PW(TT_SCALAR) SP_PW(TT_VEC3) SP_PW(TT_VEC4) SP_PW(TT_SYM3) SP_PW(TT_SYM4) SP_PW(TT_R3_3_3) SP_PW(TT_R3_3_4)
+            SP_PW(TT_R3_4_3) SP_PW(TT_R3_4_4)
+        }
 #undef SP_PW
+        g_sp_launches += 1;
+    }
 }
 
 extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double *out, int nfields, const sp_tensor_desc *tens,
@@ -512,9 +523,8 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     double *dofs = (double *)ws, *coef1 = dofs + (size_t)ndof * npts, *coef2 = coef1 + (size_t)ndof * s->MC4 * vec;
     // ---- F1: dyad projection
     sp_mark(s, st, 3);
-    for (int t = 0; t < ntens; t++) launch_pointwise<false>(types[t], targs[t], s, u, dofs, st);
+    launch_pointwise<false>(types, targs, s, u, dofs, st);
     sp_mark(s, st, 4);
-    g_sp_launches += 2 * ntens;
     // ---- F2: phi analysis (eq. 33) on the folded rows: cosine block -> a_0..a_L, sine block -> b_1..b_L
     auto phi = [&](const sp_shell::PhiMat &pm, const double *B, long sBb, double *C, long sCb) -> sp_status {
         if (pm.M <= 0 || pm.K <= 0) return SP_OK;
@@ -587,7 +597,7 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
                                   (size_t)ndof, st));
     sp_mark(s, st, 7);
     // ---- F5: recombination
-    for (int t = 0; t < ntens; t++) launch_pointwise<true>(types[t], targs[t], s, dofs, out, st);
+    launch_pointwise<true>(types, targs, s, dofs, out, st);
     sp_mark(s, st, 8);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
