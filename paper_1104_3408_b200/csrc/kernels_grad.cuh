@@ -393,11 +393,16 @@ __global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_r
     }
     __syncthreads();
     // fold: E = (P0 + P1)/2, O = (P0 - P1)/2 in place (valid region; the padding stays zero)
-    for (int i = warp; i < Nt; i += nwarps)
-        for (int k = lane; k < Nr; k += 32) {
-            const double x = P0[i * PU + k], y = P1[i * PU + k];
-            P0[i * PU + k] = 0.5 * (x + y); P1[i * PU + k] = 0.5 * (x - y);
+    {   // flat over the first Nt rows, two doubles per thread and step (the pitch PU is even)
+        double2 *A2 = reinterpret_cast<double2 *>(P0), *B2 = reinterpret_cast<double2 *>(P1);
+        const int n2v = Nt * PU / 2;
+#pragma unroll 4
+        for (int q = threadIdx.x; q < n2v; q += blockDim.x) {
+            const double2 x = A2[q], y = B2[q];
+            A2[q] = make_double2(0.5 * (x.x + y.x), 0.5 * (x.y + y.y));
+            B2[q] = make_double2(0.5 * (x.x - y.x), 0.5 * (x.y - y.y));
         }
+    }
     __syncthreads();
     for (int task = warp; task < ntasks; task += nwarps) {
         const int it_ = task / kgroups, kg = task - it_ * kgroups;
