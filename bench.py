@@ -99,12 +99,23 @@ class ClockSampler:
                 pass
             time.sleep(0.05)
 
+    def _one_smi(self):
+        try:
+            out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                 capture_output=True, text=True, timeout=10).stdout.strip()
+            if out:
+                self.rows.append([x.strip() for x in out.split(",")])
+        except Exception:
+            pass
+
     def start(self):
         self.t.start()
 
     def stop(self):
         self.stop_flag = True
         self.t.join(timeout=6)
+        if not self.rows:                      # the sampling thread got nothing (NVML unavailable): one direct reading
+            self._one_smi()
         sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
         reasons = set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]

@@ -1,0 +1,160 @@
+// d/dphi of every field with the chain rule fused (eq. 17-19; 86-90 eq. 6), REFLECTION-FOLDED.
+// FD_{Nphi} is an antisymmetric circulant, FD[j'][j] = g(j'-j), g(-d) = -g(d) (eq. 8).  With h = J/2 and, for jj = 0..h,
+//     E_jj = (u_jj + u_{J-jj})/2,   O_jj = (u_jj - u_{J-jj})/2        (u_J = u_0; O_0 = O_h = 0)
+//     Gp[j'][jj] = g(j'-jj) + g(j'+jj) (0 < jj < h), Gp[j'][0] = g(j'), Gp[j'][h] = g(j'-h);   Gm[j'][jj] = g(j'-jj) - g(j'+jj)
+// the same sums regroup to
+//     (d_phi u)[j'] = (Gm O)[j'] + (Gp E)[j'],      (d_phi u)[J-j'] = (Gm O)[j'] - (Gp E)[j'],      j' = 0..h,
+// i.e. two (h+1) x (h+1) products instead of one J x J: half the DMMAs.
+// CTA = 64 columns of one field x all rows; K (= jj) in chunks of 8 through a 3-stage cp.async pipeline holding the rows
+// u_jj and u_{J-jj} and the matching columns of Gm, Gp.  Warp (mg, ng) = MT row tiles x 2 column tiles, two accumulator
+// sets (O and E products).  Epilogue: c = d_phi u /(r sin th); with W (written by k_grad_rtheta3 into the d_x slot)
+//     d_x[j'] = cos(ph) W[j'] - sin(ph) c[j'],  d_y[j'] = sin(ph) W[j'] + cos(ph) c[j'],
+// and the same for the mirrored row J-j' (cos(ph_{J-j'}) = cos(ph_j'), sin(ph_{J-j'}) = -sin(ph_j')).
+#pragma once
+#include "kernels_gemm2.cuh"
+
+#define GF_KC 8
+#define GF_STAGES 3
+#define GF_PA 12
+#define GF_PB 68
+#define GF_PC 66
+
+template <int MT>
+__global__ void __launch_bounds__(512)
+k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, int lda, int J, int Mpad,
+                const double *__restrict__ U, long sUj, long sUb, double *__restrict__ X, double *__restrict__ Y, long sXb, int ncols,
+                PhiGradEpi ge) {
+    extern __shared__ __align__(16) double sm[];
+    const int h = J >> 1, M = h + 1, K = h + 1;
+    const int stageA = 2 * Mpad * GF_PA, stageB = 2 * GF_KC * GF_PB;
+    double *As = sm, *Bs = sm + GF_STAGES * stageA;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    const int mg = warp >> 2, ng = warp & 3;
+    const int c0 = blockIdx.x * PG_NCOL;
+    const double *Ub = U + (long)blockIdx.y * sUb + c0;
+    const int colsleft = ncols - c0;
+    const int nchunks = (K + GF_KC - 1) / GF_KC;
+    const int mtiles = (M + 7) >> 3;
+
+    auto load_chunk = [&](int kc, int st) {
+        double *as = As + st * stageA;
+        for (int q = tid; q < 2 * Mpad * 4; q += blockDim.x) {          // both matrices, 4 x 16 B per row
+            const int rr = q >> 2, hh = q & 3;
+            const int mat = rr >= Mpad, r = rr - mat * Mpad;
+            cp_async16(as + rr * GF_PA + 2 * hh, (mat ? Gp : Gm) + (long)r * lda + kc * GF_KC + 2 * hh);
+        }
+        double *bs = Bs + st * stageB;
+        for (int q = tid; q < 2 * GF_KC * (PG_NCOL / 2); q += blockDim.x) {   // rows jj and J - jj, 32 x 16 B per row
+            const int rr = q >> 5, hh = q & 31;
+            const int mir = rr >= GF_KC, r = rr - mir * GF_KC;
+            const int jj = kc * GF_KC + r;
+            int j = mir ? J - jj : jj;
+            if (j == J) j = 0;
+            double *dst = bs + rr * GF_PB + 2 * hh;
+            if (jj < K && 2 * hh < colsleft) cp_async16(dst, Ub + (long)j * sUj + 2 * hh);
+            else { dst[0] = 0.0; dst[1] = 0.0; }
+        }
+    };
+
+    double aO[MT][2][2], aE[MT][2][2];
+#pragma unroll
+    for (int a = 0; a < MT; a++)
+#pragma unroll
+        for (int b = 0; b < 2; b++) aO[a][b][0] = aO[a][b][1] = aE[a][b][0] = aE[a][b][1] = 0.0;
+
+#pragma unroll
+    for (int s = 0; s < GF_STAGES - 1; s++) {
+        if (s < nchunks) load_chunk(s, s);
+        cp_async_commit();
+    }
+    for (int kc = 0; kc < nchunks; kc++) {
+        cp_async_wait<GF_STAGES - 2>();
+        __syncthreads();
+        if (kc + GF_STAGES - 1 < nchunks) load_chunk(kc + GF_STAGES - 1, (kc + GF_STAGES - 1) % GF_STAGES);
+        cp_async_commit();
+        const double *as = As + (kc % GF_STAGES) * stageA + (mg * MT * 8 + g) * GF_PA + t;
+        const double *bs = Bs + (kc % GF_STAGES) * stageB + t * GF_PB + ng * 16 + g;
+#pragma unroll
+        for (int ks = 0; ks < GF_KC / 4; ks++) {
+            double bE[2], bO[2];
+#pragma unroll
+            for (int b = 0; b < 2; b++) {
+                const double x = bs[ks * 4 * GF_PB + b * 8], y = bs[(GF_KC + ks * 4) * GF_PB + b * 8];
+                bE[b] = 0.5 * (x + y); bO[b] = 0.5 * (x - y);
+            }
+#pragma unroll
+            for (int a = 0; a < MT; a++) {
+                if ((mg * MT + a) < mtiles) {                               // warp-uniform: skip dead row tiles
+                    const double am = as[a * 8 * GF_PA + ks * 4], ap = as[(Mpad + a * 8) * GF_PA + ks * 4];
+#pragma unroll
+                    for (int b = 0; b < 2; b++) {
+                        dmma(aO[a][b][0], aO[a][b][1], am, bO[b]);
+                        dmma(aE[a][b][0], aE[a][b][1], ap, bE[b]);
+                    }
+                }
+            }
+        }
+    }
+    // ---- epilogue, two phases.  (1) every lane scales its accumulators to c = d_phi u /(r sin th) and parks them in shared
+    // memory (the pipeline buffers are free now) as a [J][64] tile.  (2) all threads walk the tile row-contiguously: coalesced
+    // 16-byte loads of W, coalesced stores of d_x and d_y, many independent loads in flight per thread.
+    cp_async_wait<0>();
+    __syncthreads();
+    double *cs = sm;                                                        // [J][GF_PC]
+    {
+        double f[2][2];
+#pragma unroll
+        for (int b = 0; b < 2; b++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const int c = c0 + ng * 16 + b * 8 + 2 * t + e;            // flat (k, i) column: c = k + Nr i
+                const int i = c / ge.Nr, k = c - i * ge.Nr;
+                f[b][e] = (c < ncols) ? __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i) : 0.0;
+            }
+#pragma unroll
+        for (int a = 0; a < MT; a++) {
+            const int row = (mg * MT + a) * 8 + g;                          // j' in [0, h]
+            if (row >= M) continue;
+            const bool mirrored = row > 0 && row < h;
+#pragma unroll
+            for (int b = 0; b < 2; b++) {
+                const int col = ng * 16 + b * 8 + 2 * t;
+                *reinterpret_cast<double2 *>(cs + row * GF_PC + col) =
+                    make_double2((aO[a][b][0] + aE[a][b][0]) * f[b][0], (aO[a][b][1] + aE[a][b][1]) * f[b][1]);
+                if (mirrored)
+                    *reinterpret_cast<double2 *>(cs + (J - row) * GF_PC + col) =
+                        make_double2((aO[a][b][0] - aE[a][b][0]) * f[b][0], (aO[a][b][1] - aE[a][b][1]) * f[b][1]);
+            }
+        }
+    }
+    __syncthreads();
+    double *Xb = X + (long)blockIdx.y * sXb + c0, *Yb = Y + (long)blockIdx.y * sXb + c0;
+    const int npair = min(PG_NCOL, colsleft) >> 1;                          // column pairs of this tile
+    constexpr int UNR = 4;
+    for (int q0 = tid; q0 < J * 32; q0 += UNR * blockDim.x) {
+        double2 w[UNR];
+        int row[UNR], cp2[UNR];
+        bool ok[UNR];
+#pragma unroll
+        for (int z = 0; z < UNR; z++) {
+            const int q = q0 + z * blockDim.x;
+            row[z] = q >> 5; cp2[z] = q & 31;
+            ok[z] = q < J * 32 && cp2[z] < npair;
+            if (ok[z]) w[z] = *reinterpret_cast<const double2 *>(Xb + (long)row[z] * sUj + 2 * cp2[z]);
+        }
+#pragma unroll
+        for (int z = 0; z < UNR; z++) {
+            if (!ok[z]) continue;
+            const double2 c = *reinterpret_cast<const double2 *>(cs + row[z] * GF_PC + 2 * cp2[z]);
+            const double sp = __ldg(ge.sin_p + row[z]), cp = __ldg(ge.cos_p + row[z]);
+            *reinterpret_cast<double2 *>(Xb + (long)row[z] * sUj + 2 * cp2[z]) = make_double2(cp * w[z].x - sp * c.x, cp * w[z].y - sp * c.y);
+            *reinterpret_cast<double2 *>(Yb + (long)row[z] * sUj + 2 * cp2[z]) = make_double2(sp * w[z].x + cp * c.x, sp * w[z].y + cp * c.y);
+        }
+    }
+}
+
+static inline size_t gradfold_smem_bytes(int Mpad, int J) {
+    const size_t pipe = (size_t)GF_STAGES * ((size_t)2 * Mpad * GF_PA + 2 * GF_KC * GF_PB) * sizeof(double);
+    const size_t tile = (size_t)J * GF_PC * sizeof(double);                 // the epilogue tile reuses the pipeline buffers
+    return pipe > tile ? pipe : tile;
+}

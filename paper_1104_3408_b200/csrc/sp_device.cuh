@@ -31,6 +31,10 @@ struct sp_shell {
     int Np8 = 0;                  // K of d/dphi (Np) rounded up to 8
     // folded Fourier matrices (phi -> 2 pi - phi reflection, see k_pointwise): cosine / sine blocks of analysis and synthesis
     struct PhiMat { double *d = nullptr; int M = 0, K = 0, K8 = 0, MT = 0, mg = 0, Mpad = 0; };
+    // folded d/dphi operator (k_phi_grad_fold): Gm, Gp [gf_Mpad][gf_lda]
+    double *d_gm = nullptr, *d_gp = nullptr;
+    int gf_Mpad = 0, gf_lda = 0, gf_mg = 0;
+    bool gf_ok = false;
     PhiMat m_ac, m_as, m_sc, m_ss;   // analysis cos [L+1][J/2+1], sin [L][J/2-1]; synthesis cos [J/2+1][L+1], sin [J/2-1][L]
     double *d_inv_r = nullptr, *d_sin_t = nullptr, *d_cos_t = nullptr, *d_inv_sin_t = nullptr, *d_sin_p = nullptr,
            *d_cos_p = nullptr;     // Jacobian / triad factors                          (eq. 6, 51)

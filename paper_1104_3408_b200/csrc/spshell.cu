@@ -4,6 +4,7 @@
 #include "sp_internal.h"
 #include "sp_device.cuh"
 #include "kernels_gemm2.cuh"
+#include "kernels_gradphi.cuh"
 
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -62,7 +63,7 @@ extern "C" sp_status sp_shell_create(int Nr, int Nt, int Np, double rin, double 
 }
 
 static void free_dev(sp_shell *s) {
-    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_fd3p, &s->m_ac.d, &s->m_as.d, &s->m_sc.d, &s->m_ss.d, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
+    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_fd3p, &s->d_gm, &s->d_gp, &s->m_ac.d, &s->m_as.d, &s->m_sc.d, &s->m_ss.d, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
                     &s->d_inv_sin_t, &s->d_sin_p, &s->d_cos_p};
     for (auto q : p) {
         if (*q) cudaFree(*q);
@@ -134,6 +135,20 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
         for (int i = 0; i < Np; i++)
             for (int j = 0; j < Np; j++) a[(size_t)i * s->Np8 + j] = H.g3[((i - j) % Np + Np) % Np];
         if ((st = upload(&s->d_fd3p, a.data(), a.size())) != SP_OK) return st;
+        {   // folded d/dphi operator: Gm[j'][jj] = g(j'-jj) - g(j'+jj), Gp[j'][jj] = g(j'-jj) + g(j'+jj) (ends: g(j'), g(j'-h))
+            const int hh = Np / 2, M = hh + 1, mt = (M + 7) / 8;
+            s->gf_mg = (mt + 3) / 4; s->gf_Mpad = s->gf_mg * 32; s->gf_lda = round_up(M, 8);
+            auto gg = [&](int d) { return H.g3[((d % Np) + Np) % Np]; };
+            std::vector<double> gm((size_t)s->gf_Mpad * s->gf_lda, 0.0), gp(gm.size(), 0.0);
+            for (int jp = 0; jp < M; jp++)
+                for (int jj = 0; jj < M; jj++) {
+                    const bool end = (jj == 0 || jj == hh);
+                    gm[(size_t)jp * s->gf_lda + jj] = end ? 0.0 : gg(jp - jj) - gg(jp + jj);
+                    gp[(size_t)jp * s->gf_lda + jj] = end ? gg(jp - jj) : gg(jp - jj) + gg(jp + jj);
+                }
+            if ((st = upload(&s->d_gm, gm.data(), gm.size())) != SP_OK) return st;
+            if ((st = upload(&s->d_gp, gp.data(), gp.size())) != SP_OK) return st;
+        }
         const int MC = s->MC, h = Nt;                 // h = J/2
         auto mk = [&](sp_shell::PhiMat &pm, int M, int K, auto entry) -> sp_status {
             PhiTiling tl = phi_tiling(M > 0 ? M : 1);
@@ -276,6 +291,11 @@ sp_status sp_configure_kernels(sp_shell *s) {
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
     {
+        const size_t gfs = gradfold_smem_bytes(s->gf_Mpad, s->Np);
+        s->gf_ok = s->gf_mg >= 1 && s->gf_mg <= 4 && gfs <= 227 * 1024;
+        if (s->gf_ok) SP_CUDA(cudaFuncSetAttribute(k_phi_grad_fold<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gfs));
+    }
+    {
         PhiTiling tg = phi_tiling(s->Np);
         const size_t pgg = phi_smem_bytes(tg, s->Np);
         s->grad_split_ok = pgg <= 227 * 1024 && tg.mgroups <= 4;
@@ -361,9 +381,18 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         sp_mark(s, st, 1);
         PhiGradEpi ge = {du + (size_t)nf * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
-        sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, du, plane, (long)s->npts, (int)plane, nf,
-                                      st, &ge);
-        if (e != SP_OK) return e;
+        const int tiles_x = ((int)plane + PG_NCOL - 1) / PG_NCOL;
+        // the fold halves the DMMAs but doubles the rows each warp finishes; measured: it wins from Nphi = 128 upwards
+        if (s->gf_ok && Np >= 128) {      // reflection-folded d/dphi with the chain rule in the epilogue
+            const dim3 gridf(tiles_x, nf);
+            k_phi_grad_fold<4><<<gridf, s->gf_mg * 4 * 32, gradfold_smem_bytes(s->gf_Mpad, s->Np), st>>>(
+                s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge);
+            if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
+        } else {
+            sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, du, plane, (long)s->npts, (int)plane, nf,
+                                          st, &ge);
+            if (e != SP_OK) return e;
+        }
         sp_mark(s, st, 2);
         s->grad_swapped = true;
         return SP_OK;
