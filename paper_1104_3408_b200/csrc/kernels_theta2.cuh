@@ -3,7 +3,7 @@
 // CTA = (component, m, block of 36 radii).  K (= latitude ii) is walked in chunks of 16 through a 3-stage
 // cp.async pipeline holding the F^n_m rows (and F^{-n}_m for complex components) and the raw coefficient
 // rows a_m, b_m (real) or a^r, b^r, a^i, b^i (complex) of the CTA's radii.
-// Warp (mg, ng): MT latitude tiles x 3 column tiles; a column tile is 4 radii x {v = 0, 1} interleaved
+// Warp (mg, ng): MT latitude tiles x NT column tiles; a column tile is 4 radii x {v = 0, 1} interleaved
 // (col = 2k + v), so a lane's accumulator pair is the (v=0, v=1) pair of one radius:
 //   real (n = 0):  v=0: a~_m = F^0_m a_m,  v=1: b~_m = F^0_m b_m
 //   complex spin n, m > 0 (reading Q12, F^n_{-m} = F^{-n}_m by eq. 47):
@@ -14,9 +14,7 @@
 #pragma once
 #include "kernels_gemm2.cuh"
 
-#define TH_NT 3
-#define TH_NGC 3
-#define TH_RC (TH_NGC * TH_NT * 4)     // 36 radii per CTA
+#define TH_RC 36                        // radii per CTA = 9 column tiles = NT tiles per warp x (9 / NT) warp columns
 #define TH_PKB 37
 #define TH_KC 16
 #define TH_STAGES 3
@@ -32,8 +30,11 @@ struct ThetaComp2 { int dof; int n; };
 struct ThetaBatch2 { ThetaComp2 c[SP_THETA2_BATCH]; };
 
 // F2: [7][L+1][Nt8][Nt8] zero padded
-template <int MT, bool CPLX>
-__global__ void __launch_bounds__(512, 1)
+// NT = column tiles per warp: 3 (3 warp columns, 72 accumulator registers for complex components) or 1 (9 warp columns,
+// three times as many warps with a third of the registers).  Which one is faster depends on the grid; sp_build_matrices
+// times both on the device and keeps the winner.
+template <int MT, int NT, bool CPLX>
+__global__ void __launch_bounds__(NT == 3 ? 512 : 896, 1)
 k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt8, int Nr, int MC4, int mgroups,
          const double *__restrict__ coef, double *__restrict__ cout) {
     extern __shared__ __align__(16) double sm[];
@@ -78,13 +79,13 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
         }
     };
 
-    double acc[NMAT][MT][TH_NT][2];
+    double acc[NMAT][MT][NT][2];
 #pragma unroll
     for (int x = 0; x < NMAT; x++)
 #pragma unroll
         for (int a = 0; a < MT; a++)
 #pragma unroll
-            for (int b = 0; b < TH_NT; b++) acc[x][a][b][0] = acc[x][a][b][1] = 0.0;
+            for (int b = 0; b < NT; b++) acc[x][a][b][0] = acc[x][a][b][1] = 0.0;
 
 #pragma unroll
     for (int s = 0; s < TH_STAGES - 1; s++) {
@@ -104,10 +105,10 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
         const double *bs = Bs + (kc % TH_STAGES) * stageB;
 #pragma unroll
         for (int ks = 0; ks < TH_KC / 4; ks++) {
-            double b1[TH_NT], b2[TH_NT];
+            double b1[NT], b2[NT];
 #pragma unroll
-            for (int b = 0; b < TH_NT; b++) {
-                const int kk = (ng * TH_NT + b) * 4 + kq;
+            for (int b = 0; b < NT; b++) {
+                const int kk = (ng * NT + b) * 4 + kq;
                 const double x = bs[(arrX * TH_KC + ks * 4 + t) * TH_PKB + kk];
                 if (CPLX) {
                     const double y = ysgn * bs[(arrY * TH_KC + ks * 4 + t) * TH_PKB + kk];
@@ -121,11 +122,11 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
             for (int a = 0; a < MT; a++) {
                 const double a1 = as[a * 8 * TH_PA + ks * 4];
 #pragma unroll
-                for (int b = 0; b < TH_NT; b++) dmma(acc[0][a][b][0], acc[0][a][b][1], a1, b1[b]);
+                for (int b = 0; b < NT; b++) dmma(acc[0][a][b][0], acc[0][a][b][1], a1, b1[b]);
                 if (CPLX) {
                     const double a2 = as[(Nt8 + a * 8) * TH_PA + ks * 4];
 #pragma unroll
-                    for (int b = 0; b < TH_NT; b++) dmma(acc[NMAT - 1][a][b][0], acc[NMAT - 1][a][b][1], a2, b2[b]);
+                    for (int b = 0; b < NT; b++) dmma(acc[NMAT - 1][a][b][0], acc[NMAT - 1][a][b][1], a2, b2[b]);
                 }
             }
         }
@@ -137,8 +138,8 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
         const int i = (mg * MT + a) * 8 + g;
         if (i >= Nt) continue;
 #pragma unroll
-        for (int b = 0; b < TH_NT; b++) {
-            const int kl = (ng * TH_NT + b) * 4 + t;
+        for (int b = 0; b < NT; b++) {
+            const int kl = (ng * NT + b) * 4 + t;
             if (kl >= nrad) continue;
             const size_t off = (size_t)i * Nr + k0 + kl;
             const double pp = acc[0][a][b][0], qq = acc[0][a][b][1];

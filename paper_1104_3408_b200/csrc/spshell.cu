@@ -221,6 +221,46 @@ extern "C" sp_status sp_get_matrix(const sp_shell *s, int which, int n, int m, d
 #include "kernels_theta2.cuh"
 #include "kernels_wave.cuh"
 
+// theta step launcher: NT = 3 or 1 column tiles per warp (see kernels_theta2.cuh)
+static void theta2_tiling(const sp_shell *s, int NT, int &MT, int &mgroups) {
+    const int mtiles = s->Nt8 / 8, ngc = 9 / NT;
+    MT = (mtiles % 3 == 0) ? 3 : (mtiles % 4 == 0) ? 4 : (mtiles < 3 ? mtiles : 3);
+    if (((mtiles + MT - 1) / MT) * ngc > (NT == 3 ? 16 : 28) && mtiles % 4 == 0) MT = 4;
+    mgroups = (mtiles + MT - 1) / MT;
+}
+static bool theta2_fits(const sp_shell *s, int NT) {
+    int MT, mg;
+    theta2_tiling(s, NT, MT, mg);
+    return mg * (9 / NT) <= (NT == 3 ? 16 : 28) && theta2_smem_bytes(s->Nt8, true) <= 227 * 1024;
+}
+static sp_status launch_theta2(const sp_shell *s, int NT, const std::vector<ThetaComp2> &rl, const std::vector<ThetaComp2> &cx,
+                               const double *coef1, double *coef2, cudaStream_t st) {
+    int MT, mgroups;
+    theta2_tiling(s, NT, MT, mgroups);
+    const dim3 block(mgroups * (9 / NT) * 32);
+    const int gz = (s->Nr + TH_RC - 1) / TH_RC;
+    for (int pass = 0; pass < 2; pass++) {
+        const std::vector<ThetaComp2> &lst = pass ? cx : rl;
+        const size_t sm = theta2_smem_bytes(s->Nt8, pass == 1);
+        for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
+            ThetaBatch2 b;
+            const int nb = (int)std::min<size_t>(SP_THETA2_BATCH, lst.size() - c0);
+            for (int q = 0; q < nb; q++) b.c[q] = lst[c0 + q];
+            const dim3 grid(s->L + 1, nb, gz);
+#define SP_TH2(MTV, NTV)                                                                                                        \
+    if (pass) k_theta2<MTV, NTV, true><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, coef1, coef2); \
+    else k_theta2<MTV, NTV, false><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, coef1, coef2);
+#define SP_TH2M(NTV)                                                                                     \
+    switch (MT) { case 1: SP_TH2(1, NTV) break; case 2: SP_TH2(2, NTV) break; case 3: SP_TH2(3, NTV) break; default: SP_TH2(4, NTV) break; }
+            if (NT == 3) { SP_TH2M(3) } else { SP_TH2M(1) }
+#undef SP_TH2M
+#undef SP_TH2
+            g_sp_launches += 1;
+        }
+    }
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
 static size_t grad_smem_bytes(const sp_shell *s) {
     return ((size_t)2 * s->Nt8 * s->PU + (size_t)s->Nr8 * s->PU + 2 * s->Nt) * sizeof(double);
 }
@@ -305,17 +345,43 @@ sp_status sp_configure_kernels(sp_shell *s) {
             SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
         }
     }
-    if (s->Nt8 / 8 <= 20) {
+    s->theta_NT = 0;
+    if (theta2_smem_bytes(s->Nt8, true) <= 227 * 1024) {
         const int t1 = (int)theta2_smem_bytes(s->Nt8, false), t2 = (int)theta2_smem_bytes(s->Nt8, true);
-        if (t2 > 227 * 1024) return SP_ERR_UNSUPPORTED;
-        SP_CUDA(cudaFuncSetAttribute(k_theta2<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));
-        SP_CUDA(cudaFuncSetAttribute(k_theta2<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));
-        SP_CUDA(cudaFuncSetAttribute(k_theta2<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));
-        SP_CUDA(cudaFuncSetAttribute(k_theta2<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));
-        SP_CUDA(cudaFuncSetAttribute(k_theta2<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
-        SP_CUDA(cudaFuncSetAttribute(k_theta2<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
-        SP_CUDA(cudaFuncSetAttribute(k_theta2<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
-        SP_CUDA(cudaFuncSetAttribute(k_theta2<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
+#define SP_TA(MTV, NTV)                                                                                           \
+    SP_CUDA(cudaFuncSetAttribute(k_theta2<MTV, NTV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));    \
+    SP_CUDA(cudaFuncSetAttribute(k_theta2<MTV, NTV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
+        SP_TA(1, 3) SP_TA(2, 3) SP_TA(3, 3) SP_TA(4, 3) SP_TA(1, 1) SP_TA(2, 1) SP_TA(3, 1) SP_TA(4, 1)
+#undef SP_TA
+        // measure, don't guess: time both warp tilings on scratch data shaped like a GHG state (12 real + 18 complex
+        // components = 48 coefficient arrays) and keep the winner
+        const bool ok3 = theta2_fits(s, 3), ok1 = theta2_fits(s, 1);
+        if (ok3 && !ok1) s->theta_NT = 3;
+        else if (ok1 && !ok3) s->theta_NT = 1;
+        else if (ok1 && ok3) {
+            const size_t dofsz = (size_t)s->MC4 * s->Nt * s->Nr;
+            double *scr = nullptr;
+            const int nscr = 48;
+            if (cudaMalloc((void **)&scr, 2 * nscr * dofsz * sizeof(double)) != cudaSuccess) { cudaGetLastError(); s->theta_NT = 3; return SP_OK; }
+            SP_CUDA(cudaMemset(scr, 0, 2 * nscr * dofsz * sizeof(double)));
+            std::vector<ThetaComp2> rl, cx;
+            for (int q = 0; q < 12; q++) rl.push_back({q, 0});
+            for (int q = 0; q < 18; q++) cx.push_back({12 + 2 * q, 1 + q % 3});
+            cudaEvent_t e0, e1;
+            SP_CUDA(cudaEventCreate(&e0)); SP_CUDA(cudaEventCreate(&e1));
+            float best[2] = {1e30f, 1e30f};
+            for (int rep = 0; rep < 4; rep++)
+                for (int v = 0; v < 2; v++) {
+                    cudaEventRecord(e0);
+                    launch_theta2(s, v ? 1 : 3, rl, cx, scr, scr + nscr * dofsz, 0);
+                    cudaEventRecord(e1);
+                    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(scr); return SP_ERR_CUDA; }
+                    float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+                    if (rep > 0 && ms < best[v]) best[v] = ms;
+                }
+            cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(scr);
+            s->theta_NT = best[1] < best[0] ? 1 : 3;
+        }
     }
     return SP_OK;
 }
@@ -573,34 +639,11 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     // ---- F3: per-(n,m) theta matrices (eq. 62)
     {
         const int mtiles = s->Nt8 / 8;
-        const int MT = (mtiles % 3 == 0) ? 3 : (mtiles % 4 == 0) ? 4 : (mtiles < 3 ? mtiles : 3);
-        const int mgroups = (mtiles + MT - 1) / MT;
-        if (mgroups * TH_NGC <= 16) {
+        if (s->theta_NT > 0) {
             std::vector<ThetaComp2> rl, cx;
             for (const ThetaComp &c : comps) (c.cplx ? cx : rl).push_back({c.dof, c.n});
-            const dim3 block(mgroups * TH_NGC * 32);
-            const int gz = (Nr + TH_RC - 1) / TH_RC;
-            for (int pass = 0; pass < 2; pass++) {
-                const std::vector<ThetaComp2> &lst = pass ? cx : rl;
-                const size_t sm = theta2_smem_bytes(s->Nt8, pass == 1);
-                for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
-                    ThetaBatch2 b;
-                    const int nb = (int)std::min<size_t>(SP_THETA2_BATCH, lst.size() - c0);
-                    for (int q = 0; q < nb; q++) b.c[q] = lst[c0 + q];
-                    const dim3 grid(s->L + 1, nb, gz);
-#define SP_TH2(MTV)                                                                                                          \
-    if (pass) k_theta2<MTV, true><<<grid, block, sm, st>>>(b, s->d_F, s->L, Nt, s->Nt8, Nr, s->MC4, mgroups, coef1, coef2);   \
-    else k_theta2<MTV, false><<<grid, block, sm, st>>>(b, s->d_F, s->L, Nt, s->Nt8, Nr, s->MC4, mgroups, coef1, coef2);
-                    switch (MT) {
-                        case 1: SP_TH2(1) break;
-                        case 2: SP_TH2(2) break;
-                        case 3: SP_TH2(3) break;
-                        default: SP_TH2(4) break;
-                    }
-#undef SP_TH2
-                    g_sp_launches += 1;
-                }
-            }
+            sp_status e2 = launch_theta2(s, s->theta_NT, rl, cx, coef1, coef2, st);
+            if (e2 != SP_OK) return e2;
         } else {   // very large Ntheta: generic global-memory kernel
             const int nwarps = (Nr + 3) / 4;
             if (nwarps > 20) return SP_ERR_UNSUPPORTED;
