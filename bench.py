@@ -438,6 +438,21 @@ def run_ours(args):
                                       "path_frac_of_fp64_peak": f2 * w2.units / (m2 / k2 * 1e-3) * 1e-12 / peak_tf,
                                       "dominant": r2["kernel"], "dominant_frac": r2["frac"],
                                       "stages_ms": {k: v["ms"] for k, v in t2.items()}}
+            if cid == 5:      # the configuration's own workload: 200 RK4 steps with the Yn filter after every substep
+                from paper_1104_3408_b200.wave import WaveRK4, wave_dt
+                uw = torch.from_numpy(synth.wave_exact(c2, 0.0)).cuda()
+                rk = WaveRK4(w2.sh, c2["tensors"])
+                dt = wave_dt(c2["Nr"], c2["Nt"], c2["Np"], c2["rmin"], c2["rmax"])
+                rk.evolve(uw.clone(), dt, 5)
+                torch.cuda.synchronize()
+                ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                ev0.record()
+                rk.evolve(uw, dt, 200)
+                ev1.record()
+                torch.cuda.synchronize()
+                msw = ev0.elapsed_time(ev1)
+                others["config5"]["rk4_200_steps_ms"] = msw
+                others["config5"]["rk4_steps_per_s"] = 200.0 / (msw * 1e-3)
             wl = w2
         line["other_configs"] = others
     if not args.no_cpu_baseline and world == 1:

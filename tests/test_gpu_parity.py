@@ -175,3 +175,18 @@ def test_gradient_exact_polynomial_on_gpu():
     g = _grad_gpu(_shell(cfg), f[None])
     want = np.stack([(3 * x ** 2 * y - 2 * z ** 2) / 100, (x ** 3 + z) / 100, (-4 * z * x + y) / 100])[:, None]
     assert _rel(g, want) < 1e-11
+
+
+def test_scalar_Y_filter_is_the_all_scalars_layout():
+    """The paper's scalar Y-filter (the n = 0 matrices applied to every Cartesian component, ignoring the
+    tensor character) is the same call with every field declared rank 0; the graded Yg-filter (eq. 59) is that call
+    on shells created with L - d(u^mu).  Parity on config 2 data, and it must differ from the Yn result."""
+    cfg = synth.config(2)
+    u = synth.white_state(cfg, nfields=20)
+    scal = [{"rank": 0, "dims": (), "sym": (-1, -1), "fields": [f]} for f in range(20)]
+    sh = _shell(cfg)
+    got = _filt_gpu(sh, u, scal)
+    want = oracle.tensor_filter(u, cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["L"], scal)
+    assert _rel(got, want) < TOL
+    yn = _filt_gpu(sh, u, cfg["tensors"][:2])
+    assert _rel(got, yn) > 1e-3
