@@ -43,7 +43,11 @@ struct sp_shell {
     mutable bool prof = false;
     mutable cudaEvent_t ev[9] = {};
     mutable bool ev_set[9] = {};
-    mutable bool grad_swapped = false;   // last gradient ran (r,theta) kernel first, then the d/dphi GEMM
+    mutable bool grad_swapped = false;
+    // internal side stream: independent launches of one stage (real / complex theta products, ...) run concurrently,
+    // forked from and joined to the caller's stream by events
+    cudaStream_t aux = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;   // last gradient ran (r,theta) kernel first, then the d/dphi GEMM
 };
 
 // stage marks: 0 grad start, 1 after d/dphi, 2 after r-theta+chain rule, 3 filter start, 4 after projection,

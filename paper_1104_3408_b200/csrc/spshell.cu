@@ -76,6 +76,9 @@ extern "C" sp_status sp_shell_destroy(sp_shell *s) {
     free_dev(s);
     for (int q = 0; q < 9; q++)
         if (s->ev[q]) cudaEventDestroy(s->ev[q]);
+    if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+    if (s->ev_join) cudaEventDestroy(s->ev_join);
+    if (s->aux) cudaStreamDestroy(s->aux);
     delete s->host;
     delete s;
     return SP_OK;
@@ -170,6 +173,11 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
     if ((st = upload(&s->d_inv_sin_t, H.inv_sin_t.data(), Nt)) != SP_OK) return st;
     if ((st = upload(&s->d_sin_p, H.sin_p.data(), Np)) != SP_OK) return st;
     if ((st = upload(&s->d_cos_p, H.cos_p.data(), Np)) != SP_OK) return st;
+    if (!s->aux) {
+        SP_CUDA(cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking));
+        SP_CUDA(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
+        SP_CUDA(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
+    }
     if ((st = sp_configure_kernels(s)) != SP_OK) return st;
     s->built = true;
     return SP_OK;
@@ -221,6 +229,14 @@ extern "C" sp_status sp_get_matrix(const sp_shell *s, int which, int n, int m, d
 #include "kernels_theta2.cuh"
 #include "kernels_wave.cuh"
 
+// fork the side stream off the caller's stream / join it back (events; capture-safe; no host synchronisation)
+static bool sp_fork(const sp_shell *s, cudaStream_t st) {
+    return s->aux && cudaEventRecord(s->ev_fork, st) == cudaSuccess && cudaStreamWaitEvent(s->aux, s->ev_fork, 0) == cudaSuccess;
+}
+static bool sp_join(const sp_shell *s, cudaStream_t st) {
+    return cudaEventRecord(s->ev_join, s->aux) == cudaSuccess && cudaStreamWaitEvent(st, s->ev_join, 0) == cudaSuccess;
+}
+
 // theta step launcher: NT = 3 or 1 column tiles per warp (see kernels_theta2.cuh)
 static void theta2_tiling(const sp_shell *s, int NT, int &MT, int &mgroups) {
     const int mtiles = s->Nt8 / 8, ngc = 9 / NT;
@@ -239,8 +255,16 @@ static sp_status launch_theta2(const sp_shell *s, int NT, const std::vector<Thet
     theta2_tiling(s, NT, MT, mgroups);
     const dim3 block(mgroups * (9 / NT) * 32);
     const int gz = (s->Nr + TH_RC - 1) / TH_RC;
-    for (int pass = 0; pass < 2; pass++) {
+    // the real and the complex components are independent: the (shorter) real launch runs on the side stream, so CTAs of
+    // different lengths share the SMs (no lock-step fill/drain phases) and each launch fills the other's tail
+    const bool fork = s->aux && !rl.empty() && !cx.empty();
+    cudaStream_t main_st = st;
+    if (fork) {
+        if (cudaEventRecord(s->ev_fork, main_st) != cudaSuccess || cudaStreamWaitEvent(s->aux, s->ev_fork, 0) != cudaSuccess) return SP_ERR_CUDA;
+    }
+    for (int pass = 1; pass >= 0; pass--) {
         const std::vector<ThetaComp2> &lst = pass ? cx : rl;
+        st = (fork && pass == 0) ? s->aux : main_st;
         const size_t sm = theta2_smem_bytes(s->Nt8, pass == 1);
         for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
             ThetaBatch2 b;
@@ -257,6 +281,9 @@ static sp_status launch_theta2(const sp_shell *s, int NT, const std::vector<Thet
 #undef SP_TH2
             g_sp_launches += 1;
         }
+    }
+    if (fork) {
+        if (cudaEventRecord(s->ev_join, s->aux) != cudaSuccess || cudaStreamWaitEvent(main_st, s->ev_join, 0) != cudaSuccess) return SP_ERR_CUDA;
     }
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
@@ -557,8 +584,13 @@ static void launch_pointwise(const std::vector<int> &types, const std::vector<Te
     const int T = 128;
     const unsigned nb = (unsigned)(((size_t)s->Nr * s->Nt * (s->Nt + 1) + T - 1) / T);
     std::vector<char> done(types.size(), 0);
+    const cudaStream_t main_st = st;
+    bool forked = false;
+    int nlaunch = 0;
     for (size_t t0 = 0; t0 < types.size(); t0++) {
         if (done[t0]) continue;
+        // launches of different tensor groups are independent: every second one goes to the side stream
+        if ((nlaunch++ & 1) && (forked || (forked = sp_fork(s, main_st)))) st = s->aux; else st = main_st;
         TensorArgsGroup tg;                      // this tensor and the following ones of the same index structure
         int n = 0;
         for (size_t t1 = t0; t1 < types.size() && n < SP_PW_GROUP; t1++)
@@ -576,6 +608,7 @@ static void launch_pointwise(const std::vector<int> &types, const std::vector<Te
 #undef SP_PW
         g_sp_launches += 1;
     }
+    if (forked) sp_join(s, main_st);
 }
 
 extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double *out, int nfields, const sp_tensor_desc *tens,
@@ -621,20 +654,23 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     launch_pointwise<false>(types, targs, s, u, dofs, st);
     sp_mark(s, st, 4);
     // ---- F2: phi analysis (eq. 33) on the folded rows: cosine block -> a_0..a_L, sine block -> b_1..b_L
-    auto phi = [&](const sp_shell::PhiMat &pm, const double *B, long sBb, double *C, long sCb) -> sp_status {
+    auto phi = [&](const sp_shell::PhiMat &pm, const double *B, long sBb, double *C, long sCb, cudaStream_t sx) -> sp_status {
         if (pm.M <= 0 || pm.K <= 0) return SP_OK;
         PhiTiling tl = {pm.MT, pm.mg, pm.Mpad};
-        sp_status e = launch_phi_gemm(pm.d, pm.K8, pm.M, tl, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, ndof, st);
+        sp_status e = launch_phi_gemm(pm.d, pm.K8, pm.M, tl, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, ndof, sx);
         if (e == SP_ERR_UNSUPPORTED)      // odd strides: generic global-memory kernel (same padded matrix)
-            e = launch_gemm_cols<false>(pm.d, pm.K8, pm.M, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, ndof, st);
+            e = launch_gemm_cols<false>(pm.d, pm.K8, pm.M, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, ndof, sx);
         g_sp_launches += 1;
         return e;
     };
     const long cst = (long)(s->MC4 * vec);
-    sp_status e = phi(s->m_ac, dofs, (long)npts, coef1, cst);
+    // the cosine and the sine block are independent: the sine block runs on the side stream
+    bool fk = s->m_as.M > 0 && s->m_as.K > 0 && sp_fork(s, st);
+    sp_status e = phi(s->m_ac, dofs, (long)npts, coef1, cst, st);
     if (e != SP_OK) return e;
-    e = phi(s->m_as, dofs + (size_t)(Nt + 1) * vec, (long)npts, coef1 + (size_t)(s->L + 1) * vec, cst);
+    e = phi(s->m_as, dofs + (size_t)(Nt + 1) * vec, (long)npts, coef1 + (size_t)(s->L + 1) * vec, cst, fk ? s->aux : st);
     if (e != SP_OK) return e;
+    if (fk && !sp_join(s, st)) return SP_ERR_CUDA;
     sp_mark(s, st, 5);
     // ---- F3: per-(n,m) theta matrices (eq. 62)
     {
@@ -660,10 +696,12 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     }
     sp_mark(s, st, 6);
     // ---- F4: phi synthesis (eq. 31) into the folded rows: e_j (cosine block), o_j (sine block)
-    e = phi(s->m_sc, coef2, cst, dofs, (long)npts);
+    fk = s->m_ss.M > 0 && s->m_ss.K > 0 && sp_fork(s, st);
+    e = phi(s->m_sc, coef2, cst, dofs, (long)npts, st);
     if (e != SP_OK) return e;
-    e = phi(s->m_ss, coef2 + (size_t)(s->L + 1) * vec, cst, dofs + (size_t)(Nt + 1) * vec, (long)npts);
+    e = phi(s->m_ss, coef2 + (size_t)(s->L + 1) * vec, cst, dofs + (size_t)(Nt + 1) * vec, (long)npts, fk ? s->aux : st);
     if (e != SP_OK) return e;
+    if (fk && !sp_join(s, st)) return SP_ERR_CUDA;
     if (s->m_ss.K <= 0 && Nt > 1)      // L = 0: no sine modes survive, the odd rows o_j are zero
         SP_CUDA(cudaMemset2DAsync(dofs + (size_t)(Nt + 1) * vec, npts * sizeof(double), 0, (size_t)(Nt - 1) * vec * sizeof(double),
                                   (size_t)ndof, st));
