@@ -172,6 +172,52 @@ def oracle_sample(cfg, u, threads):
     return per_unit, tg + tf, desc
 
 
+def paper_style_cpu_gradient(cfg, u, threads):
+    """The paper's own CPU formulation of the derivative (eq. 13-19): one dgemm per direction on the
+    whole state array with explicit transposes, in double precision through numpy/BLAS, then the chain rule (eq. 6).
+    A timing baseline of the harness (not the oracle, not the product); returns seconds for the gradient of all fields."""
+    import numpy as np
+    from threadpoolctl import threadpool_limits
+    Nr, Nt, Np = cfg["Nr"], cfg["Nt"], cfg["Np"]
+    nv = u.shape[0]
+    k = np.arange(Nr)
+    x = -np.cos(np.pi * k / (Nr - 1))
+    c = np.where((k == 0) | (k == Nr - 1), 2.0, 1.0)
+    with np.errstate(divide="ignore"):
+        CD = (c[:, None] / c[None, :]) * (-1.0) ** (k[:, None] + k[None, :]) / (x[:, None] - x[None, :])
+    CD[k, k] = 0.0
+    CD[k, k] = -CD.sum(axis=1)
+    CD *= 2.0 / (cfg["rmax"] - cfg["rmin"])
+
+    def FD(n):
+        i = np.arange(n)
+        d = i[:, None] - i[None, :]
+        with np.errstate(divide="ignore"):
+            M = (-1.0) ** d / (2.0 * np.tan(d * np.pi / n))
+        M[i, i] = 0.0
+        return M
+    F2, F3 = FD(2 * Nt)[:Nt], FD(Np)
+    r = 0.5 * (cfg["rmax"] + cfg["rmin"]) + 0.5 * (cfg["rmax"] - cfg["rmin"]) * x
+    th = np.pi * (np.arange(Nt) + 0.5) / Nt
+    ph = 2 * np.pi * np.arange(Np) / Np
+    st, ct, sp, cp = np.sin(th)[None, :, None], np.cos(th)[None, :, None], np.sin(ph)[:, None, None], np.cos(ph)[:, None, None]
+    ir = (1.0 / r)[None, None, :]
+    with threadpool_limits(limits=threads):
+        a = time.perf_counter()
+        U = u.reshape(nv, Np, Nt, Nr)
+        dr = (U.reshape(-1, Nr) @ CD.T).reshape(U.shape)                           # eq. 13: contiguous direction
+        ext = np.concatenate([U, np.roll(U, Nt, axis=1)[:, :, ::-1, :]], axis=2)   # double cover (PAPER.md:72)
+        T = np.ascontiguousarray(ext.transpose(0, 1, 3, 2))                        # transpose, eq. 14-16
+        dth = np.ascontiguousarray((T.reshape(-1, 2 * Nt) @ F2.T).reshape(nv, Np, Nr, Nt).transpose(0, 1, 3, 2))
+        T = np.ascontiguousarray(U.transpose(0, 2, 3, 1))                          # transpose, eq. 17-19
+        dph = np.ascontiguousarray((T.reshape(-1, Np) @ F3.T).reshape(nv, Nt, Nr, Np).transpose(0, 3, 1, 2))
+        out = np.empty((3,) + U.shape)
+        out[0] = st * cp * dr + ct * cp * ir * dth - sp / st * ir * dph
+        out[1] = st * sp * dr + ct * sp * ir * dth + cp / st * ir * dph
+        out[2] = ct * dr - st * ir * dth
+        return time.perf_counter() - a, out
+
+
 def run_reference(args):
     import numpy as np
     import synth
@@ -285,6 +331,41 @@ class GpuWorkload:
         e1.record()
         torch.cuda.synchronize()
         return e0.elapsed_time(e1)
+
+    def time_call(self, which, steps, warmup=3):
+        """Device time (ms per call) of ONE of the two hot calls alone, back to back on the current stream."""
+        torch = self.torch
+
+        def one():
+            u = self.u[self.it % self.nsets]
+            self.it += 1
+            if which == "gradient":
+                self.sh.cartesian_gradient(u, out=self.du, workspace=self.ws_g)
+            else:
+                self.sh.tensor_filter(u, self.cfg["tensors"], out=self.fu, workspace=self.ws_f, descs=self.descs)
+        for _ in range(warmup):
+            one()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            one()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps
+
+    def calls_report(self, steps, peak_tf):
+        """each call alone -- units/s, achieved algorithmic TFLOP/s, fraction of the FP64 peak."""
+        fl = flops_per_unit(self.cfg)
+        fg = fl["grad_dphi"] + fl["grad_rtheta"]
+        ff = fl["filt_analysis"] + fl["filt_theta"] + fl["filt_synthesis"]
+        out = {}
+        for which, f in (("gradient", fg), ("filter", ff)):
+            ms = self.time_call(which, steps)
+            tf = f * self.units / (ms * 1e-3) * 1e-12
+            out[which] = {"ms": ms, "value": self.units / (ms * 1e-3), "algorithmic_flops_per_unit": f, "tflops": tf,
+                          "frac_of_fp64_peak": tf / peak_tf}
+        return out
 
     def stage_times(self, reps=5):
         """Per-stage device times (ms), median over reps, from CUDA events recorded inside the library
@@ -441,6 +522,8 @@ def run_ours(args):
                  "hbm_min_bytes_per_unit": 48, "stages": table},
         "fp64_peak_tflops": {"dmma": peak_tf, "dfma": probe_fp64_peak(1)},
     }
+    line["calls"] = wl.calls_report(max(10, args.steps // 4), peak_tf)
+    wl_units = wl.units
     if not args.no_others and world == 1:
         others = {}
         for cid in (2, 4, 5):
@@ -462,6 +545,10 @@ def run_ours(args):
                                       "path_frac_of_fp64_peak": f2 * w2.units / (m2 / k2 * 1e-3) * 1e-12 / peak_tf,
                                       "dominant": r2["kernel"], "dominant_frac": r2["frac"],
                                       "stages_ms": {k: v["ms"] for k, v in t2.items()}}
+            others[f"config{cid}"]["calls"] = w2.calls_report(max(10, k2 // 4), peak_tf)
+            if cid in (2, 5):  # these states fit L2: the figure above rotates inputs (HBM-cold); this one re-reads one copy
+                w2.nsets = 1
+                others[f"config{cid}"]["ms_per_step_l2_warm"] = w2.time_steps(k2, 3) / k2
             if cid == 5:      # the configuration's own workload: 200 RK4 steps with the Yn filter after every substep
                 from paper_1104_3408_b200.wave import WaveRK4, wave_dt
                 uw = torch.from_numpy(synth.wave_exact(c2, 0.0)).cuda()
@@ -476,14 +563,35 @@ def run_ours(args):
                 torch.cuda.synchronize()
                 msw = ev0.elapsed_time(ev1)
                 others["config5"]["rk4_200_steps_ms"] = msw
-                others["config5"]["rk4_steps_per_s"] = 200.0 / (msw * 1e-3)
+                ug = torch.from_numpy(synth.wave_exact(c2, 0.0)).cuda()
+                rk.evolve(ug, dt, 2, graph=True)                 # captures the step for this state array
+                ug.copy_(torch.from_numpy(synth.wave_exact(c2, 0.0)))
+                torch.cuda.synchronize()
+                ev0.record()
+                rk.evolve(ug, dt, 200, graph=True)
+                ev1.record()
+                torch.cuda.synchronize()
+                msg = ev0.elapsed_time(ev1)
+                others["config5"]["rk4_200_steps_graph_ms"] = msg
+                others["config5"]["rk4_steps_per_s"] = 200.0 / (min(msw, msg) * 1e-3)
             wl = w2
         line["other_configs"] = others
     if not args.no_cpu_baseline and world == 1:
         threads = os.cpu_count() or 1
         pu, wall, desc = oracle_sample(cfg, synth.make_state(cfg), threads)
+        pu1, _, _ = oracle_sample(cfg, synth.make_state(cfg), 1)
         line["cpu_baseline"] = {"value": 1.0 / pu, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
-                                "seconds": wall}
+                                "seconds": wall, "value_1_thread": 1.0 / pu1}
+        # the paper's own CPU formulation of the derivative (dgemm + transposes, double precision), 1 thread and all threads
+        uh = synth.make_state(cfg)
+        paper_style_cpu_gradient(cfg, uh, threads)
+        t1 = min(paper_style_cpu_gradient(cfg, uh, 1)[0] for _ in range(2))
+        tn = min(paper_style_cpu_gradient(cfg, uh, threads)[0] for _ in range(2))
+        line["cpu_paper_style"] = {
+            "what": "gradient only: numpy/BLAS dgemm per direction with explicit transposes (PAPER.md:135-168), double precision",
+            "unit": "grid-point*fields/s (gradient call alone; compare with calls.gradient.value)",
+            "value_1_thread": wl_units / t1, "value_all_threads": wl_units / tn, "cores": threads,
+            "paper_context": "PAPER.md Tab. 4: GTX580 vs one i7-870 core 10.0x / 16.7x / 21.8x for the whole time step"}
     else:
         line["cpu_baseline"] = None
     print(json.dumps(line))

@@ -104,6 +104,15 @@ sp_status sp_rhs_first_order_wave(const sp_shell *shell, const double *u_dev, do
 /* y <- a*x + b*y over n doubles (the RK4 combination steps of config 5). */
 sp_status sp_axpby(double a, const double *x_dev, double b, double *y_dev, size_t n, void *cuda_stream);
 
+/* One combination step of the classical RK4 scheme over n doubles, u and k read once:
+ *     acc_out   = acc_in + c_acc * k
+ *     stage_out = u + c_stage * k            (skipped when stage_out is NULL)
+ * All pointers are device pointers owned by the caller.  acc_out may equal acc_in or u (the last stage writes the new
+ * state over u); acc_in may equal u (the first stage).  stage_out must be distinct from every other array and acc_out
+ * from k, else SP_ERR_INVALID_ARG.  Asynchronous on cuda_stream, allocates nothing. */
+sp_status sp_rk4_stage(const double *u_dev, const double *k_dev, const double *acc_in_dev, double *acc_out_dev,
+                       double *stage_out_dev, double c_acc, double c_stage, size_t n, void *cuda_stream);
+
 /* Copy one host-built matrix out (for tests).  which: 0 = CD^ (Nr x Nr), 1 = FD_{2Ntheta} upper half
  * (Ntheta x 2Ntheta), 2 = FD_{Nphi} (Nphi x Nphi), 3 = Fourier analysis rows (2L+1 x Nphi; row 0 = a_0,
  * row 2m-1 = a_m, row 2m = b_m), 4 = Fourier synthesis (Nphi x 2L+1, same column order),

@@ -8,7 +8,7 @@ _lib = None
 # every symbol include/spshell.h declares
 EXPORTED_SYMBOLS = [
     "sp_shell_create", "sp_shell_destroy", "sp_build_matrices", "sp_workspace_bytes", "sp_cartesian_gradient",
-    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_axpby", "sp_get_matrix", "sp_probe_fp64_peak",
+    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_axpby", "sp_rk4_stage", "sp_get_matrix", "sp_probe_fp64_peak",
     "sp_status_string", "sp_profile_enable", "sp_profile_read", "sp_launch_count",
 ]
 
@@ -45,6 +45,8 @@ def lib():
                                        C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rhs_first_order_wave.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_axpby.argtypes = [C.c_double, C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sp_rk4_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_size_t,
+                                   C.c_void_p]
         L.sp_get_matrix.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.sp_probe_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.sp_profile_enable.argtypes = [C.c_void_p, C.c_int]
@@ -210,3 +212,14 @@ class Shell:
         _dev_f64(x, "x"); _dev_f64(y, "y")
         _check(lib().sp_axpby(float(a), x.data_ptr(), float(b), y.data_ptr(), y.numel(), _stream_ptr(stream)), "sp_axpby")
         return y
+
+    @staticmethod
+    def rk4_stage(u, k, acc_in, acc_out, stage_out, c_acc, c_stage, stream=None):
+        """acc_out <- acc_in + c_acc k;  stage_out <- u + c_stage k (skipped if stage_out is None)."""
+        for t, nm in ((u, "u"), (k, "k"), (acc_in, "acc_in"), (acc_out, "acc_out")):
+            _dev_f64(t, nm)
+        if stage_out is not None:
+            _dev_f64(stage_out, "stage_out")
+        _check(lib().sp_rk4_stage(u.data_ptr(), k.data_ptr(), acc_in.data_ptr(), acc_out.data_ptr(),
+                                  stage_out.data_ptr() if stage_out is not None else None, float(c_acc), float(c_stage),
+                                  u.numel(), _stream_ptr(stream)), "sp_rk4_stage")

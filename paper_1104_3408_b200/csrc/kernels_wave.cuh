@@ -40,6 +40,19 @@ __global__ void __launch_bounds__(256) k_axpby(double a, const double *__restric
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) y[q] = a * x[q] + b * y[q];
 }
 
+// One RK4 combination: acc_out = acc_in + c_acc * k  and, if stage_out is given, stage_out = u + c_stage * k.
+// u and k are read once; acc_out may alias acc_in or u (same index read before written by the same thread).
+__global__ void __launch_bounds__(256) k_rk4_stage(const double *u, const double *__restrict__ k, const double *acc_in,
+                                                   double *acc_out, double *stage_out, double c_acc, double c_stage, size_t n) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) {
+        const double kq = k[q], uq = u[q];
+        const double a = (acc_in == u) ? uq : acc_in[q];
+        if (stage_out) stage_out[q] = c_stage * kq + uq;
+        acc_out[q] = c_acc * kq + a;
+    }
+}
+
 // ---- FP64 issue-peak probes (register-only loops)
 __global__ void k_probe_dmma(double *out, int iters, double a, double b) {
     double c[8][2];

@@ -737,6 +737,19 @@ extern "C" sp_status sp_axpby(double a, const double *x, double b, double *y, si
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
 
+extern "C" sp_status sp_rk4_stage(const double *u, const double *k, const double *acc_in, double *acc_out, double *stage_out,
+                                  double c_acc, double c_stage, size_t n, void *stream) {
+    if (!u || !k || !acc_in || !acc_out) return SP_ERR_INVALID_ARG;
+    if (stage_out == u || stage_out == k || stage_out == acc_in || (stage_out && stage_out == acc_out) || acc_out == k)
+        return SP_ERR_INVALID_ARG;
+    if (n == 0) return SP_OK;
+    size_t nb = (n + 255) / 256;
+    if (nb > 148 * 16) nb = 148 * 16;
+    g_sp_launches += 1;
+    k_rk4_stage<<<(unsigned)nb, 256, 0, (cudaStream_t)stream>>>(u, k, acc_in, acc_out, stage_out, c_acc, c_stage, n);
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
 extern "C" sp_status sp_probe_fp64_peak(int mode, double *tflops) {
     if (!tflops || mode < 0 || mode > 1) return SP_ERR_INVALID_ARG;
     cudaDeviceProp prop;

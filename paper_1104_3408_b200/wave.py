@@ -28,6 +28,7 @@ class WaveRK4:
         _, f, w = shell.workspace_bytes(5)
         self.ws_w = torch.empty(w // 8, dtype=torch.float64, device=dev)
         self.ws_f = torch.empty(f // 8, dtype=torch.float64, device=dev)
+        self._graph, self._graph_key = None, None
 
     def _filter(self, v):
         self.sh.tensor_filter(v, self.tensors, out=v, workspace=self.ws_f, descs=self.descs)
@@ -35,22 +36,42 @@ class WaveRK4:
     def _rhs(self, v):
         self.sh.rhs_first_order_wave(v, out=self.k, workspace=self.ws_w)
 
-    def evolve(self, u, dt, nsteps):
-        """u: CUDA tensor [5, Np, Nt, Nr], advanced in place by nsteps RK4 steps; returns u."""
-        ax = self.sh.axpby
+    def _step(self, u, dt):
+        st = self.sh.rk4_stage
+        self._rhs(u)                                                      # k1
+        st(u, self.k, u, self.acc, self.stage, dt / 6.0, 0.5 * dt); self._filter(self.stage)
+        self._rhs(self.stage)                                             # k2
+        st(u, self.k, self.acc, self.acc, self.stage, dt / 3.0, 0.5 * dt); self._filter(self.stage)
+        self._rhs(self.stage)                                             # k3
+        st(u, self.k, self.acc, self.acc, self.stage, dt / 3.0, dt); self._filter(self.stage)
+        self._rhs(self.stage)                                             # k4
+        st(u, self.k, self.acc, u, None, dt / 6.0, 0.0)                   # new state written over u
         self._filter(u)
+
+    def evolve(self, u, dt, nsteps, graph=False):
+        """u: CUDA tensor [5, Np, Nt, Nr], advanced in place by nsteps RK4 steps; returns u.
+        graph=True captures one RK4 step (4 RHS, 4 filters, 4 combinations: every pointer is fixed) in a CUDA graph and
+        replays it nsteps times: the step is ~50 short launches, so the replay removes their launch gaps."""
+        import torch
+        self._filter(u)
+        if graph and nsteps > 0:
+            key = (u.data_ptr(), float(dt))
+            if self._graph_key != key:
+                side = torch.cuda.Stream()
+                side.wait_stream(torch.cuda.current_stream())
+                with torch.cuda.stream(side):
+                    keep = u.clone()
+                    self._step(u, dt)                                     # warm-up outside capture
+                    u.copy_(keep)
+                torch.cuda.current_stream().wait_stream(side)
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g):
+                    self._step(u, dt)
+                u.copy_(keep)                                             # capture does not execute, but keep the state explicit
+                self._graph, self._graph_key = g, key
+            for _ in range(nsteps):
+                self._graph.replay()
+            return u
         for _ in range(nsteps):
-            self._rhs(u)                                   # k1
-            self.acc.copy_(u); ax(dt / 6.0, self.k, 1.0, self.acc)
-            self.stage.copy_(u); ax(0.5 * dt, self.k, 1.0, self.stage); self._filter(self.stage)
-            self._rhs(self.stage)                          # k2
-            ax(dt / 3.0, self.k, 1.0, self.acc)
-            self.stage.copy_(u); ax(0.5 * dt, self.k, 1.0, self.stage); self._filter(self.stage)
-            self._rhs(self.stage)                          # k3
-            ax(dt / 3.0, self.k, 1.0, self.acc)
-            self.stage.copy_(u); ax(dt, self.k, 1.0, self.stage); self._filter(self.stage)
-            self._rhs(self.stage)                          # k4
-            ax(dt / 6.0, self.k, 1.0, self.acc)
-            u.copy_(self.acc)
-            self._filter(u)
+            self._step(u, dt)
         return u
