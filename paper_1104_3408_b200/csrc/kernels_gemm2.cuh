@@ -1,21 +1,22 @@
 // phi-direction contraction, shared-memory staged (the hot GEMM: d/dphi, phi analysis, phi synthesis).
 //     C[b][m][c] = sum_k A[m][k] * B[b][k][c],   B[b][k][c] = B + b*sBb + k*sBk + c  (columns contiguous)
 // (eq. 17-19 without the transposes; 254-259 eq. 33; 243-246 eq. 31.)
-// CTA tile = ALL rows of A x 64 columns; K walked in chunks of 16 through a 3-stage cp.async pipeline:
-//   As[stage][Mpad][20]  (pitch 20 doubles: fragment reads hit 16 distinct 8-byte banks)
-//   Bs[stage][16][68]    (pitch 68 = 4 mod 16: likewise)
-// Warp (mg, ng): MT m-tiles x 2 n-tiles of 8x8, DMMA.8x8x4.  Requires even strides / ncols and 16-byte
+// CTA tile = ALL rows of A x NC columns (NC = 64; 32 when the 64-wide grid would leave SMs idle or with a single CTA: small
+// states, see phi_ncol); K walked in chunks of 16 through a 3-stage cp.async pipeline:
+//   As[stage][Mpad][20]    (pitch 20 doubles: fragment reads hit 16 distinct 8-byte banks)
+//   Bs[stage][16][NC + 4]  (pitch = 4 mod 16: likewise)
+// Warp (mg, ng): MT m-tiles x 2 n-tiles of 8x8, DMMA.8x8x4; NC/16 warps along the columns.  Requires even strides / ncols and 16-byte
 // aligned bases (checked by the launcher; otherwise the generic kernel of kernels_gemm.cuh is used).
 #pragma once
 #include "sp_device.cuh"
 
 #include <cstdint>
+#include <cstdlib>
 
 #define PG_NCOL 64
 #define PG_KC 16
 #define PG_STAGES 3
 #define PG_PA 20
-#define PG_PB 68
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
     unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -33,21 +34,21 @@ struct PhiGradEpi {
     const double *inv_r, *inv_sin_t, *sin_p, *cos_p;
     int Nr;
 };
-#define PG_PW 72
 
-template <int MT, bool EPI_GRAD>
-__global__ void __launch_bounds__(512)
+template <int MT, bool EPI_GRAD, int NC>
+__global__ void __launch_bounds__(NC * 8)
 k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const double *__restrict__ B, long sBk, long sBb,
            double *__restrict__ C, long sCm, long sCb, int ncols, PhiGradEpi ge) {
     extern __shared__ __align__(16) double sm[];
     // plain products: K chunks of 16, 3 stages; gradient variant (which also holds the W tile): chunks of 8, 4 stages
     constexpr int KC = EPI_GRAD ? 8 : 16, STG = EPI_GRAD ? 4 : 3, PA = KC + 4;
+    constexpr int PG_PB = NC + 4, PG_PW = NC + 8, NG = NC / 16, HC = NC / 2;
     const int stageA = Mpad * PA, stageB = KC * PG_PB;
     double *As = sm, *Bs = sm + STG * stageA;
     double *Ws = Bs + STG * stageB;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-    const int mg = warp >> 2, ng = warp & 3;
-    const int c0 = blockIdx.x * PG_NCOL;
+    const int mg = warp / NG, ng = warp % NG;
+    const int c0 = blockIdx.x * NC;
     const double *Bb = B + (long)blockIdx.y * sBb + c0;
     double *Cb = C + (long)blockIdx.y * sCb + c0;
     const int nchunks = (K + KC - 1) / KC;
@@ -62,8 +63,8 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
         }
         // B chunk: 8 rows x 64 columns (32 x 16 B per row); rows >= K and columns >= ncols are zero-filled
         double *bs = Bs + st * stageB;
-        for (int q = tid; q < KC * (PG_NCOL / 2); q += blockDim.x) {
-            const int r = q >> 5, h = q & 31;
+        for (int q = tid; q < KC * HC; q += blockDim.x) {
+            const int r = q / HC, h = q % HC;
             const int k = kc * KC + r;
             double *dst = bs + r * PG_PB + 2 * h;
             if (k < K && 2 * h < colsleft) cp_async16(dst, Bb + (long)k * sBk + 2 * h);
@@ -78,8 +79,8 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
         for (int b = 0; b < 2; b++) acc[a][b][0] = acc[a][b][1] = 0.0;
 
     if (EPI_GRAD) {      // oldest cp.async group: complete long before the epilogue
-        for (int q = tid; q < M * (PG_NCOL / 2); q += blockDim.x) {
-            const int r = q >> 5, h = q & 31;
+        for (int q = tid; q < M * HC; q += blockDim.x) {
+            const int r = q / HC, h = q % HC;
             if (2 * h < colsleft) cp_async16(Ws + r * PG_PW + 2 * h, Cb + (long)r * sCm + 2 * h);
         }
         cp_async_commit();
@@ -168,9 +169,18 @@ static inline PhiTiling phi_tiling(int M) {
     best.Mpad = best.mgroups * best.MT * 8;
     return best;
 }
-static inline size_t phi_smem_bytes(const PhiTiling &tl, int Mgrad = 0) {
+static inline size_t phi_smem_bytes(const PhiTiling &tl, int Mgrad = 0, int NC = PG_NCOL) {
     const int KC = Mgrad ? 8 : 16, STG = Mgrad ? 4 : 3, PA = KC + 4;
-    return ((size_t)STG * ((size_t)tl.Mpad * PA + KC * PG_PB) + (size_t)Mgrad * PG_PW) * sizeof(double);
+    return ((size_t)STG * ((size_t)tl.Mpad * PA + KC * (NC + 4)) + (size_t)Mgrad * (NC + 8)) * sizeof(double);
+}
+// column tile width: 64, or 32 when 64-wide tiles would give fewer than 2 CTAs per SM (small states: more, smaller CTAs keep
+// every SM busy and let several CTAs per SM overlap their load, product and store phases).  SP_PHI_NC overrides (experiments).
+extern int g_sp_num_sms;
+static inline int phi_ncol(int ncols, int nbatch) {
+    static const int forced = [] { const char *e = getenv("SP_PHI_NC"); return e ? atoi(e) : 0; }();
+    if (forced == 32 || forced == 64) return forced;
+    const long ctas64 = (long)((ncols + 63) / 64) * nbatch;
+    return ctas64 < 2L * g_sp_num_sms ? 32 : 64;
 }
 
 // returns SP_ERR_UNSUPPORTED when the fast-path preconditions do not hold (caller falls back)
@@ -180,24 +190,29 @@ static sp_status launch_phi_gemm(const double *A, int lda, int M, const PhiTilin
     if ((sBk | sBb | sCm | sCb | (long)ncols) & 1) return SP_ERR_UNSUPPORTED;
     if (((uintptr_t)B | (uintptr_t)C) & 15) return SP_ERR_UNSUPPORTED;
     if (tl.mgroups > 4) return SP_ERR_UNSUPPORTED;
-    dim3 grid((ncols + PG_NCOL - 1) / PG_NCOL, nbatch), block(tl.mgroups * 4 * 32);
+    const int NC = phi_ncol(ncols, nbatch);
+    dim3 grid((ncols + NC - 1) / NC, nbatch), block(tl.mgroups * (NC / 16) * 32);
+#define SP_PG(MTV, EPIV, SM, GE)                                                                                              \
+    if (NC == 32) k_phi_gemm<MTV, EPIV, 32><<<grid, block, SM, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, GE); \
+    else k_phi_gemm<MTV, EPIV, 64><<<grid, block, SM, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, GE);
     if (ge) {
         if ((ge->sYb & 1) || ((uintptr_t)ge->Y & 15)) return SP_ERR_UNSUPPORTED;
-        const size_t sm = phi_smem_bytes(tl, M);
+        const size_t sm = phi_smem_bytes(tl, M, NC);
         if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;
         switch (tl.MT) {
-            case 4: k_phi_gemm<4, true><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, *ge); break;
-            case 5: k_phi_gemm<5, true><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, *ge); break;
-            default: k_phi_gemm<6, true><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, *ge); break;
+            case 4: SP_PG(4, true, sm, *ge) break;
+            case 5: SP_PG(5, true, sm, *ge) break;
+            default: SP_PG(6, true, sm, *ge) break;
         }
         return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
     }
-    const size_t sm = phi_smem_bytes(tl);
+    const size_t sm = phi_smem_bytes(tl, 0, NC);
     PhiGradEpi none = {};
     switch (tl.MT) {
-        case 4: k_phi_gemm<4, false><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, none); break;
-        case 5: k_phi_gemm<5, false><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, none); break;
-        default: k_phi_gemm<6, false><<<grid, block, sm, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, none); break;
+        case 4: SP_PG(4, false, sm, none) break;
+        case 5: SP_PG(5, false, sm, none) break;
+        default: SP_PG(6, false, sm, none) break;
     }
+#undef SP_PG
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }

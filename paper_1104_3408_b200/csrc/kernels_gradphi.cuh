@@ -5,7 +5,7 @@
 // the same sums regroup to
 //     (d_phi u)[j'] = (Gm O)[j'] + (Gp E)[j'],      (d_phi u)[J-j'] = (Gm O)[j'] - (Gp E)[j'],      j' = 0..h,
 // i.e. two (h+1) x (h+1) products instead of one J x J: half the DMMAs.
-// CTA = 64 columns of one field x all rows; K (= jj) in chunks of 8 through a 3-stage cp.async pipeline holding the rows
+// CTA = NC (64, or 32 for small states: phi_ncol) columns of one field x all rows; K (= jj) in chunks of 8 through a 3-stage cp.async pipeline holding the rows
 // u_jj and u_{J-jj} and the matching columns of Gm, Gp.  Warp (mg, ng) = MT row tiles x 2 column tiles, two accumulator
 // sets (O and E products).  Epilogue: c = d_phi u /(r sin th); with W (written by k_grad_rtheta3 into the d_x slot)
 //     d_x[j'] = cos(ph) W[j'] - sin(ph) c[j'],  d_y[j'] = sin(ph) W[j'] + cos(ph) c[j'],
@@ -16,21 +16,20 @@
 #define GF_KC 8
 #define GF_STAGES 3
 #define GF_PA 12
-#define GF_PB 68
-#define GF_PC 66
 
-template <int MT>
-__global__ void __launch_bounds__(512)
+template <int MT, int NC>
+__global__ void __launch_bounds__(NC * 8)
 k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, int lda, int J, int Mpad,
                 const double *__restrict__ U, long sUj, long sUb, double *__restrict__ X, double *__restrict__ Y, long sXb, int ncols,
                 PhiGradEpi ge) {
     extern __shared__ __align__(16) double sm[];
+    constexpr int GF_PB = NC + 4, GF_PC = NC + 2, NG = NC / 16, HC = NC / 2;
     const int h = J >> 1, M = h + 1, K = h + 1;
     const int stageA = 2 * Mpad * GF_PA, stageB = 2 * GF_KC * GF_PB;
     double *As = sm, *Bs = sm + GF_STAGES * stageA;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-    const int mg = warp >> 2, ng = warp & 3;
-    const int c0 = blockIdx.x * PG_NCOL;
+    const int mg = warp / NG, ng = warp % NG;
+    const int c0 = blockIdx.x * NC;
     const double *Ub = U + (long)blockIdx.y * sUb + c0;
     const int colsleft = ncols - c0;
     const int nchunks = (K + GF_KC - 1) / GF_KC;
@@ -44,8 +43,8 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
             cp_async16(as + rr * GF_PA + 2 * hh, (mat ? Gp : Gm) + (long)r * lda + kc * GF_KC + 2 * hh);
         }
         double *bs = Bs + st * stageB;
-        for (int q = tid; q < 2 * GF_KC * (PG_NCOL / 2); q += blockDim.x) {   // rows jj and J - jj, 32 x 16 B per row
-            const int rr = q >> 5, hh = q & 31;
+        for (int q = tid; q < 2 * GF_KC * HC; q += blockDim.x) {   // rows jj and J - jj, NC/2 x 16 B per row
+            const int rr = q / HC, hh = q % HC;
             const int mir = rr >= GF_KC, r = rr - mir * GF_KC;
             const int jj = kc * GF_KC + r;
             int j = mir ? J - jj : jj;
@@ -129,17 +128,17 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
     }
     __syncthreads();
     double *Xb = X + (long)blockIdx.y * sXb + c0, *Yb = Y + (long)blockIdx.y * sXb + c0;
-    const int npair = min(PG_NCOL, colsleft) >> 1;                          // column pairs of this tile
+    const int npair = min(NC, colsleft) >> 1;                          // column pairs of this tile
     constexpr int UNR = 4;
-    for (int q0 = tid; q0 < J * 32; q0 += UNR * blockDim.x) {
+    for (int q0 = tid; q0 < J * HC; q0 += UNR * blockDim.x) {
         double2 w[UNR];
         int row[UNR], cp2[UNR];
         bool ok[UNR];
 #pragma unroll
         for (int z = 0; z < UNR; z++) {
             const int q = q0 + z * blockDim.x;
-            row[z] = q >> 5; cp2[z] = q & 31;
-            ok[z] = q < J * 32 && cp2[z] < npair;
+            row[z] = q / HC; cp2[z] = q % HC;
+            ok[z] = q < J * HC && cp2[z] < npair;
             if (ok[z]) w[z] = *reinterpret_cast<const double2 *>(Xb + (long)row[z] * sUj + 2 * cp2[z]);
         }
 #pragma unroll
@@ -153,8 +152,8 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
     }
 }
 
-static inline size_t gradfold_smem_bytes(int Mpad, int J) {
-    const size_t pipe = (size_t)GF_STAGES * ((size_t)2 * Mpad * GF_PA + 2 * GF_KC * GF_PB) * sizeof(double);
-    const size_t tile = (size_t)J * GF_PC * sizeof(double);                 // the epilogue tile reuses the pipeline buffers
+static inline size_t gradfold_smem_bytes(int Mpad, int J, int NC = PG_NCOL) {
+    const size_t pipe = (size_t)GF_STAGES * ((size_t)2 * Mpad * GF_PA + 2 * GF_KC * (NC + 4)) * sizeof(double);
+    const size_t tile = (size_t)J * (NC + 2) * sizeof(double);                 // the epilogue tile reuses the pipeline buffers
     return pipe > tile ? pipe : tile;
 }

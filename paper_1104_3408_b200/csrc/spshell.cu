@@ -21,6 +21,7 @@
         if (e_ != cudaSuccess) return SP_ERR_CUDA;   \
     } while (0)
 
+int g_sp_num_sms = 148;
 unsigned long long g_sp_launches = 0;
 
 static int round_up(int a, int b) { return (a + b - 1) / b * b; }
@@ -352,24 +353,32 @@ sp_status sp_configure_kernels(sp_shell *s) {
             }
         }
     }
+    g_sp_num_sms = s->num_sms;
     PhiTiling tmax = {6, 4, 4 * 6 * 8};
     const int pg = (int)phi_smem_bytes(tmax);
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+#define SP_PGA(MTV)                                                                                             \
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, false, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg)); \
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, false, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    SP_PGA(4) SP_PGA(5) SP_PGA(6)
+#undef SP_PGA
     {
         const size_t gfs = gradfold_smem_bytes(s->gf_Mpad, s->Np);
         s->gf_ok = s->gf_mg >= 1 && s->gf_mg <= 4 && gfs <= 227 * 1024;
-        if (s->gf_ok) SP_CUDA(cudaFuncSetAttribute(k_phi_grad_fold<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gfs));
+        if (s->gf_ok) {
+            SP_CUDA(cudaFuncSetAttribute(k_phi_grad_fold<4, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gfs));
+            SP_CUDA(cudaFuncSetAttribute(k_phi_grad_fold<4, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gfs));
+        }
     }
     {
         PhiTiling tg = phi_tiling(s->Np);
         const size_t pgg = phi_smem_bytes(tg, s->Np);
         s->grad_split_ok = pgg <= 227 * 1024 && tg.mgroups <= 4;
         if (s->grad_split_ok) {
-            SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
-            SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<5, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
-            SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<6, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
+#define SP_PGA(MTV)                                                                                                  \
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg)); \
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
+            SP_PGA(4) SP_PGA(5) SP_PGA(6)
+#undef SP_PGA
         }
     }
     s->theta_NT = 0;
@@ -474,11 +483,15 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         sp_mark(s, st, 1);
         PhiGradEpi ge = {du + (size_t)nf * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
-        const int tiles_x = ((int)plane + PG_NCOL - 1) / PG_NCOL;
         // the fold halves the DMMAs but doubles the rows each warp finishes; measured: it wins from Nphi = 128 upwards
         if (s->gf_ok && Np >= 128) {      // reflection-folded d/dphi with the chain rule in the epilogue
-            const dim3 gridf(tiles_x, nf);
-            k_phi_grad_fold<4><<<gridf, s->gf_mg * 4 * 32, gradfold_smem_bytes(s->gf_Mpad, s->Np), st>>>(
+            const int NC = phi_ncol((int)plane, nf);
+            const dim3 gridf(((int)plane + NC - 1) / NC, nf);
+            if (NC == 32)
+                k_phi_grad_fold<4, 32><<<gridf, s->gf_mg * 2 * 32, gradfold_smem_bytes(s->gf_Mpad, s->Np, 32), st>>>(
+                    s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge);
+            else
+                k_phi_grad_fold<4, 64><<<gridf, s->gf_mg * 4 * 32, gradfold_smem_bytes(s->gf_Mpad, s->Np), st>>>(
                 s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge);
             if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         } else {
