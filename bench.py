@@ -442,15 +442,23 @@ def roofline_for(cfg, stages_ms, units, peak_tf, hbm_gbs, hbm_src):
         table[k] = {"ms": ms, "tflops": fl[k] * units / (ms * 1e-3) * 1e-12}
     dom = max(table, key=lambda k: table[k]["ms"])
     ach = table[dom]["tflops"]
-    traffic = None
+    traffic, executed = None, {}
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(f"config{cfg['id']}", {}).get(dom)
+            tj = json.load(open(tp))
+            traffic = tj.get(f"config{cfg['id']}", {}).get(dom)
+            executed = tj.get(f"config{cfg['id']}_executed_flops", {})
         except Exception:
-            traffic = None
+            traffic, executed = None, {}
+    for k in table:                      # executed (ncu instruction counts, profiles/) next to the algorithmic count
+        if k in executed:
+            table[k]["executed_tflops"] = executed[k] / (table[k]["ms"] * 1e-3) * 1e-12
     roof = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
             "traffic": traffic,
+            "achieved_executed": table[dom].get("executed_tflops"),
+            "frac_executed": (table[dom]["executed_tflops"] / peak_tf) if "executed_tflops" in table[dom] else None,
+            "executed_flops_per_step": sum(executed.values()) if executed else None,
             "peak_source": "FP64 DMMA issue peak measured live by sp_probe_fp64_peak (148 SMs x 64 FMA/clk x 2 x 1.965 GHz = 37.2 nominal)",
             "hbm_gbs": hbm_gbs, "hbm_source": hbm_src}
     return roof, table
@@ -519,8 +527,13 @@ def run_ours(args):
         "roofline": roof,
         "path": {"algorithmic_flops_per_unit": tot_fl, "tflops": tot_fl * wl.units / (ms / args.steps * 1e-3) * 1e-12,
                  "frac_of_fp64_peak": tot_fl * wl.units / (ms / args.steps * 1e-3) * 1e-12 / peak_tf,
-                 "hbm_min_bytes_per_unit": 48, "stages": table},
+                 "hbm_min_bytes_per_unit": 48, "stages": table,
+                 "executed_tflops": (roof["executed_flops_per_step"] / (ms / args.steps * 1e-3) * 1e-12)
+                 if roof.get("executed_flops_per_step") else None,
+                 "note": "algorithmic = dense products as the paper defines them (SURVEY.md 8(d)); executed = FP64 instructions counted "
+                         "by ncu (profiles/): the reflection folds execute fewer flops than the algorithmic count"},
         "fp64_peak_tflops": {"dmma": peak_tf, "dfma": probe_fp64_peak(1)},
+        "kernel_variants": wl.sh.tuning(),
     }
     line["calls"] = wl.calls_report(max(10, args.steps // 4), peak_tf)
     wl_units = wl.units

@@ -131,6 +131,12 @@ sp_status sp_probe_fp64_peak(int mode, double *tflops_out);
 sp_status sp_profile_enable(sp_shell *shell, int on);
 sp_status sp_profile_read(const sp_shell *shell, double *ms7_host);
 
+/* Kernel variants sp_build_matrices selected for this shell (reporting only): out[0] = column tiles per warp of the theta
+ * kernel (3 or 1, chosen by a timing run at build; 0 = generic kernel), out[1] = radial tiles per warp task of the
+ * (r,theta) gradient kernel (3 or 5), out[2] = 1 if d/dphi uses the reflection-folded kernel, out[3] = 2 if the
+ * double-buffered variant of the persistent (r,theta) kernel fits (it is used by calls with at least three waves of planes).  SP_ERR_NOT_BUILT before sp_build_matrices. */
+sp_status sp_get_tuning(const sp_shell *shell, int out[4]);
+
 /* Number of kernels the hot calls have launched since the library was loaded (host-side counter). */
 unsigned long long sp_launch_count(void);
 

@@ -8,7 +8,7 @@ _lib = None
 # every symbol include/spshell.h declares
 EXPORTED_SYMBOLS = [
     "sp_shell_create", "sp_shell_destroy", "sp_build_matrices", "sp_workspace_bytes", "sp_cartesian_gradient",
-    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_axpby", "sp_rk4_stage", "sp_get_matrix", "sp_probe_fp64_peak",
+    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_axpby", "sp_rk4_stage", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
     "sp_status_string", "sp_profile_enable", "sp_profile_read", "sp_launch_count",
 ]
 
@@ -47,6 +47,7 @@ def lib():
         L.sp_axpby.argtypes = [C.c_double, C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rk4_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_size_t,
                                    C.c_void_p]
+        L.sp_get_tuning.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
         L.sp_get_matrix.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.sp_probe_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.sp_profile_enable.argtypes = [C.c_void_p, C.c_int]
@@ -137,6 +138,12 @@ class Shell:
         return out
 
     STAGES = ("grad_dphi", "grad_rtheta", "filt_project", "filt_analysis", "filt_theta", "filt_synthesis", "filt_recombine")
+
+    def tuning(self):
+        """Kernel variants chosen at build time (sp_get_tuning)."""
+        out = (C.c_int * 4)()
+        _check(lib().sp_get_tuning(self._h, out), "sp_get_tuning")
+        return {"theta_NT": out[0], "grad_KT": out[1], "dphi_folded": bool(out[2]), "grad_plane_buffers": out[3]}
 
     def profile(self, on=True):
         _check(lib().sp_profile_enable(self._h, 1 if on else 0), "sp_profile_enable")

@@ -219,3 +219,48 @@ def test_misaligned_buffers_take_the_general_path():
     # and the aligned fast path gives the same numbers to rounding
     fast = sh.cartesian_gradient(torch.from_numpy(u).cuda()).cpu().numpy()
     assert _rel(fast, got) < TOL
+
+
+def test_bench_launch_configuration_two_streams():
+    """The step exactly as bench.py times it (config 3, pre-allocated outputs and workspaces, gradient and filter of
+    one state issued on two CUDA streams, several steps in flight): bit-identical to the same calls on one stream, and
+    sampled against the oracle."""
+    import bench
+    torch = _torch()
+    cfg = synth.config(3)
+    wl = bench.GpuWorkload(cfg, nsets=2)
+    wl.step()
+    torch.cuda.synchronize()
+    du1, fu1 = wl.du.clone(), wl.fu.clone()                  # serial, input set 0
+    wl.it = 0
+    sg, sf = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for _ in range(4):                                       # sets 0, 1, 0, 1 back to back: the pipeline is full
+        wl.step(sg, sf)
+    wl.it = 0
+    wl.step(sg, sf)                                          # ends on set 0
+    torch.cuda.synchronize()
+    assert torch.equal(wl.du, du1) and torch.equal(wl.fu, fu1)
+    u = wl.u_host
+    got = wl.du.cpu().numpy()
+    rng = np.random.default_rng(33)
+    ns = 500
+    samp = np.stack([rng.integers(cfg["Nr"], size=ns), rng.integers(cfg["Nt"], size=ns), rng.integers(cfg["Np"], size=ns),
+                     rng.integers(cfg["nfields"], size=ns)], axis=1).astype(np.int32)
+    want = oracle.gradient_at(u, cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["rmin"], cfg["rmax"], samp)
+    fmax = np.max(np.abs(got.reshape(3, cfg["nfields"], -1)), axis=2)
+    for s, (k, i, j, mu) in enumerate(samp):
+        assert np.all(np.abs(got[:, mu, j, i, k] - want[s]) <= TOL * fmax[:, mu])
+    k = 11
+    wantf = oracle.tensor_filter(u, cfg["Nr"], cfg["Nt"], cfg["Np"], cfg["L"], cfg["tensors"], ksel=k)
+    assert _rel(wl.fu.cpu().numpy()[..., k:k + 1], wantf[..., k:k + 1]) < TOL
+
+
+def test_gradient_is_deterministic():
+    torch = _torch()
+    cfg = synth.config(2)
+    sh = _shell(cfg)
+    u = torch.from_numpy(synth.white_state(cfg)).cuda()
+    a = sh.cartesian_gradient(u).clone()
+    for _ in range(3):
+        assert torch.equal(sh.cartesian_gradient(u), a)
