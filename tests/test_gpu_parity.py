@@ -241,6 +241,12 @@ def test_bench_launch_configuration_two_streams():
     wl.step(sg, sf)                                          # ends on set 0
     torch.cuda.synchronize()
     assert torch.equal(wl.du, du1) and torch.equal(wl.fu, fu1)
+    wl.capture()                                             # the same step as replayed CUDA graphs (bench.py's default)
+    wl.du.zero_(); wl.fu.zero_()
+    for n in (0, 1, 0, 1, 0):
+        wl.graphs[n].replay()
+    torch.cuda.synchronize()
+    assert torch.equal(wl.du, du1) and torch.equal(wl.fu, fu1)
     u = wl.u_host
     got = wl.du.cpu().numpy()
     rng = np.random.default_rng(33)
