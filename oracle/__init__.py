@@ -210,3 +210,44 @@ def wave_rk4(u, Nr, Nt, Np, rmin, rmax, L, tensors, dt, nsteps):
         k4 = R(F(u + dt * k3))
         u = F(u + dt / 6.0 * (k1 + 2.0 * k2 + 2.0 * k3 + k4))
     return u
+
+
+# ---- GHG right-hand side (oracle/ghg_oracle.c; Appendix A) ----
+def ghg_rhs(u, du, H, dH, Nr, Nt, Np, rmin, rmax, bc_outer=False):
+    """(A.8)-(A.10) for the 50-field state u with its Cartesian gradient du [3,50], gauge source H [4] and dH [3,4];
+    bc_outer: freezing condition (A.20)-(A.21) on the shell k = Nr-1."""
+    u, nf = _state(u, Nr, Nt, Np)
+    assert nf == 50
+    du = np.ascontiguousarray(du, dtype=np.float64).reshape(3, 50, Np, Nt, Nr)
+    H = np.ascontiguousarray(H, dtype=np.float64).reshape(4, Np, Nt, Nr)
+    dH = np.ascontiguousarray(dH, dtype=np.float64).reshape(3, 4, Np, Nt, Nr)
+    out = np.empty_like(u)
+    bad = lib().orc_ghg_rhs(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), C.c_double(rmin), C.c_double(rmax), u.ctypes, du.ctypes,
+                            H.ctypes, dH.ctypes, C.c_int(1 if bc_outer else 0), out.ctypes)
+    if bad:
+        raise ValueError(f"metric not Lorentzian/invertible at {bad} points")
+    return out
+
+
+def ghg_init(g, Nr, Nt, Np, rmin, rmax):
+    """Initial data of PAPER.md:732-737 from a metric g_ab [10] with d_t g_ab = 0: d_iab = numerical gradient of g_ab,
+    k_ab by (A.6), H_a = -Gamma_a (A.18), dH = numerical gradient of H.  Returns u [50], H [4], dH [3,4]."""
+    g, nf = _state(g, Nr, Nt, Np)
+    assert nf == 10
+    u = np.zeros((50, Np, Nt, Nr))
+    u[:10] = g
+    u[20:] = gradient(g, Nr, Nt, Np, rmin, rmax).reshape(30, Np, Nt, Nr)
+    H = np.zeros((4, Np, Nt, Nr))
+    bad = lib().orc_ghg_init(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), u.ctypes, H.ctypes)
+    if bad:
+        raise ValueError(f"metric not Lorentzian/invertible at {bad} points")
+    dH = gradient(H, Nr, Nt, Np, rmin, rmax).reshape(3, 4, Np, Nt, Nr)
+    return u, H, dH
+
+
+def ghg_lapse_shift(u, Nr, Nt, Np):
+    """alpha, beta^i, gamma^{ij} (xx,xy,xz,yy,yz,zz) of (A.4)-(A.5): [10] state-shaped."""
+    u, nf = _state(u, Nr, Nt, Np)
+    out = np.zeros((10, Np, Nt, Nr))
+    lib().orc_ghg_lapse_shift(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), u.ctypes, out.ctypes)
+    return out

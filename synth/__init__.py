@@ -12,3 +12,4 @@ not a public dataset; these fields take its SHAPE and stand in for it.
 from .configs import CONFIGS, config, ghg_tensors, wave_tensors, tensor_ncomp  # noqa: F401
 from .fields import make_state, scalar_basis, white_state  # noqa: F401
 from .wave import wave_exact  # noqa: F401
+from .ghg import grid_xyz, kerr_schild_metric, minkowski_metric, perturbed_ghg_state  # noqa: F401

@@ -1,0 +1,113 @@
+"""Pins of the GHG right-hand-side oracle (oracle/ghg_oracle.c; Appendix A) against what the paper and the
+mathematics fix, none of them the oracle's own formulas retyped:
+  * the Kerr-Schild metric (A.17) is a static solution of the vacuum Einstein equations, so the RHS (A.8)-(A.10) of data
+    built from it must vanish up to the truncation error of the spectral derivatives and fall exponentially with the
+    resolution ("rhs -> round-off for static data"); a dropped term, a wrong sign or a misplaced index
+    leaves an O(1) residual that does not converge.  Checked for the centred hole and for a displaced one (no symmetry);
+  * Minkowski: exactly zero;
+  * lapse, shift, inverse 3-metric against the closed forms (A.19);
+  * boundary condition (A.20)-(A.21): the incoming characteristic fields of (A.14) are frozen, the outgoing one and
+    d_t g_ab keep the value of the unconstrained RHS.
+"""
+import numpy as np
+
+import oracle
+import synth
+
+RMIN, RMAX = 1.8, 6.8
+
+
+def _static_residual(Nr, Nt, center, bc=False):
+    Np = 2 * Nt
+    g = synth.kerr_schild_metric(Nr, Nt, Np, RMIN, RMAX, center=center)
+    u, H, dH = oracle.ghg_init(g, Nr, Nt, Np, RMIN, RMAX)
+    du = oracle.gradient(u, Nr, Nt, Np, RMIN, RMAX)
+    rhs = oracle.ghg_rhs(u, du, H, dH, Nr, Nt, Np, RMIN, RMAX, bc_outer=bc)
+    return [float(np.abs(rhs[a:b]).max()) for a, b in ((0, 10), (10, 20), (20, 50))]
+
+
+def test_kerr_schild_is_static_centred_hole_converges_exponentially():
+    res = {Nr: _static_residual(Nr, 8, (0.0, 0.0, 0.0)) for Nr in (9, 13, 17, 25)}
+    for Nr in res:
+        assert res[Nr][0] < 1e-15                       # (A.8) vanishes identically by the construction of k_ab
+    for a, b in ((9, 13), (13, 17), (17, 25)):
+        assert res[b][1] < 0.1 * res[a][1] and res[b][2] < 0.1 * res[a][2]
+    assert res[9][1] < 0.1                               # already small at 9 radial points ...
+    assert res[25][1] < 1e-7 and res[25][2] < 1e-8       # ... and at truncation level at 25
+
+
+def test_kerr_schild_is_static_displaced_hole_converges_in_r_and_angle():
+    c = (0.15, -0.1, 0.12)
+    coarse, fine_r, fine = _static_residual(11, 6, c), _static_residual(21, 6, c), _static_residual(21, 12, c)
+    assert fine[1] < 1e-5 and fine[2] < 1e-6
+    assert fine[1] < 0.05 * coarse[1] and fine[2] < 0.05 * coarse[2]
+    assert fine[1] < 0.1 * fine_r[1]                     # at Ntheta = 6 the angular error dominates; 12 removes it
+
+
+def test_static_residual_with_boundary_condition_still_converges():
+    a, b = _static_residual(13, 8, (0.0, 0.0, 0.0), bc=True), _static_residual(25, 8, (0.0, 0.0, 0.0), bc=True)
+    assert b[1] < 1e-7 and b[1] < 1e-3 * a[1]
+
+
+def test_minkowski_gives_zero():
+    Nr, Nt, Np = 7, 6, 12
+    g = synth.minkowski_metric(Nr, Nt, Np)
+    u, H, dH = oracle.ghg_init(g, Nr, Nt, Np, 1.0, 3.0)
+    assert np.abs(u[10:]).max() < 1e-13 and np.abs(H).max() < 1e-13
+    u[10:] = 0.0
+    z = np.zeros((3, 50, Np, Nt, Nr))
+    rhs = oracle.ghg_rhs(u, z, np.zeros_like(H), np.zeros_like(dH), Nr, Nt, Np, 1.0, 3.0)
+    assert np.abs(rhs).max() == 0.0
+
+
+def test_lapse_shift_inverse_metric_closed_forms_A19():
+    Nr, Nt, Np = 9, 6, 12
+    g = synth.kerr_schild_metric(Nr, Nt, Np, RMIN, RMAX)
+    u = np.zeros((50, Np, Nt, Nr)); u[:10] = g
+    out = oracle.ghg_lapse_shift(u, Nr, Nt, Np)
+    x, y, z = synth.grid_xyz(Nr, Nt, Np, RMIN, RMAX)
+    r = np.sqrt(x * x + y * y + z * z)
+    f = 2.0 / r
+    l = [x / r, y / r, z / r]
+    assert np.abs(out[0] - 1.0 / np.sqrt(1.0 + f)).max() < 1e-15
+    for i in range(3):
+        assert np.abs(out[1 + i] - l[i] * f / (1.0 + f)).max() < 1e-15
+    c = 4
+    for i in range(3):
+        for j in range(i, 3):
+            assert np.abs(out[c] - ((i == j) - f / (1.0 + f) * l[i] * l[j])).max() < 1e-15
+            c += 1
+
+
+def test_boundary_condition_freezes_incoming_characteristic_fields():
+    """(A.14): e^1 = -g + k + s^i d_i (speed alpha - b, outgoing at the outer boundary), e^2 = -g + k - s^i d_i and the two
+    tangential combinations of d_i (incoming).  With (A.20)-(A.21): d_t e^2 = 0, tangential d_t d = 0, d_t e^1 and d_t g
+    unchanged.  s_i is rebuilt here with numpy from the state's own 3-metric."""
+    Nr, Nt, Np = 9, 6, 12
+    g = synth.kerr_schild_metric(Nr, Nt, Np, RMIN, RMAX, center=(0.1, 0.05, -0.08))
+    u, H, dH = oracle.ghg_init(g, Nr, Nt, Np, RMIN, RMAX)
+    u = synth.perturbed_ghg_state(u, 1e-2, 7)
+    du = oracle.gradient(u, Nr, Nt, Np, RMIN, RMAX)
+    free = oracle.ghg_rhs(u, du, H, dH, Nr, Nt, Np, RMIN, RMAX, bc_outer=False)
+    bc = oracle.ghg_rhs(u, du, H, dH, Nr, Nt, Np, RMIN, RMAX, bc_outer=True)
+    assert np.array_equal(free[..., :Nr - 1], bc[..., :Nr - 1])            # interior untouched
+    x, y, z = synth.grid_xyz(Nr, Nt, Np, RMIN, RMAX)
+    sym = [[0, 1, 2, 3], [1, 4, 5, 6], [2, 5, 7, 8], [3, 6, 8, 9]]
+    worst = 0.0
+    for j in range(Np):
+        for i in range(Nt):
+            k = Nr - 1
+            gam = np.array([[u[sym[a + 1][b + 1], j, i, k] for b in range(3)] for a in range(3)])
+            gi = np.linalg.inv(gam)
+            l = np.array([x[j, i, k], y[j, i, k], z[j, i, k]]); l /= np.linalg.norm(l)
+            s_dn = l / np.sqrt(l @ gi @ l)
+            s_up = gi @ s_dn
+            for ab in range(10):
+                tg0, tk0, td0 = free[ab, j, i, k], free[10 + ab, j, i, k], np.array([free[20 + 10 * q + ab, j, i, k] for q in range(3)])
+                tg1, tk1, td1 = bc[ab, j, i, k], bc[10 + ab, j, i, k], np.array([bc[20 + 10 * q + ab, j, i, k] for q in range(3)])
+                scale = max(abs(tg0), abs(tk0), np.abs(td0).max(), 1e-30)
+                worst = max(worst, abs(tg1 - tg0) / scale)
+                worst = max(worst, abs((-tg1 + tk1 - s_up @ td1)) / scale)                       # incoming e^2 frozen
+                worst = max(worst, np.abs(td1 - s_dn * (s_up @ td1)).max() / scale)              # tangential part frozen
+                worst = max(worst, abs((-tg1 + tk1 + s_up @ td1) - (-tg0 + tk0 + s_up @ td0)) / scale)   # outgoing kept
+    assert worst < 1e-13
