@@ -101,6 +101,25 @@ sp_status sp_tensor_filter(const sp_shell *shell, const double *u_dev, double *o
 sp_status sp_rhs_first_order_wave(const sp_shell *shell, const double *u_dev, double *dudt_dev,
                                   void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 
+/* ---- Generalized-harmonic (GHG) Einstein system, Appendix A ----
+ * State u: 50 state-shaped fields, g_ab (tt,tx,ty,tz,xx,xy,xz,yy,yz,zz), k_ab (same ten; eq. A.6), d_iab (i = x,y,z
+ * slowest, then the same ten).  H: gauge source H_a, 4 fields; dH: its Cartesian gradient, [3][4] fields (d_x H_t, d_x H_x,
+ * ..., d_z H_z); d_t H_a = 0 (A.18).
+ *
+ * sp_rhs_ghg: dudt = right-hand side (A.8)-(A.10) with gamma0 = gamma2 = 1, gamma1 = -1, the dependent
+ * quantities (lapse, shift, inverse metrics, Christoffel symbols, nabla_a H_b) by (A.3)-(A.5), (A.11) and PAPER.md:682; the
+ * spatial derivatives of u are taken by sp_cartesian_gradient into the workspace.  bc_outer != 0: the freezing condition
+ * (A.20)-(A.21) is applied on the outer shell k = Nr-1 (s_i = outward normal x_i/r normalised with gamma^{ij}).  All
+ * pointers are device pointers owned by the caller; dudt must not alias u; workspace >= sp_ghg_workspace_bytes.
+ * Asynchronous on cuda_stream, allocates nothing.  A metric that is not Lorentzian at some point gives NaN there (no check). */
+sp_status sp_ghg_workspace_bytes(const sp_shell *shell, size_t *bytes);
+sp_status sp_rhs_ghg(const sp_shell *shell, const double *u_dev, const double *H_dev, const double *dH_dev, double *dudt_dev,
+                     int bc_outer, void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Initial data from a metric with d_t g_ab = 0: on entry u holds g_ab (fields 0..9) and d_iab (fields
+ * 20..49); fills k_ab = (beta^i/alpha) d_iab (A.6) into fields 10..19 and H_a = -Gamma_a (A.18) into H (4 fields). */
+sp_status sp_ghg_init(const sp_shell *shell, double *u_dev, double *H_dev, void *cuda_stream);
+
 /* y <- a*x + b*y over n doubles (the RK4 combination steps of config 5). */
 sp_status sp_axpby(double a, const double *x_dev, double b, double *y_dev, size_t n, void *cuda_stream);
 

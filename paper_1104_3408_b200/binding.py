@@ -8,7 +8,7 @@ _lib = None
 # every symbol include/spshell.h declares
 EXPORTED_SYMBOLS = [
     "sp_shell_create", "sp_shell_destroy", "sp_build_matrices", "sp_workspace_bytes", "sp_cartesian_gradient",
-    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_axpby", "sp_rk4_stage", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
+    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_axpby", "sp_rk4_stage", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
     "sp_status_string", "sp_profile_enable", "sp_profile_read", "sp_launch_count",
 ]
 
@@ -47,6 +47,9 @@ def lib():
         L.sp_axpby.argtypes = [C.c_double, C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rk4_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_size_t,
                                    C.c_void_p]
+        L.sp_ghg_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
+        L.sp_rhs_ghg.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sp_ghg_init.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.sp_get_tuning.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
         L.sp_get_matrix.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.sp_probe_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
@@ -212,6 +215,41 @@ class Shell:
         _check(lib().sp_rhs_first_order_wave(self._h, u.data_ptr(), out.data_ptr(), ws.data_ptr(), ws.numel() * 8,
                                              _stream_ptr(stream)), "sp_rhs_first_order_wave")
         return out
+
+    def ghg_workspace_bytes(self):
+        n = C.c_size_t()
+        _check(lib().sp_ghg_workspace_bytes(self._h, C.byref(n)), "sp_ghg_workspace_bytes")
+        return n.value
+
+    def rhs_ghg(self, u, H, dH, out=None, bc_outer=True, workspace=None, stream=None):
+        """GHG right-hand side (A.8)-(A.10) of the 50-field state u [50, Np, Nt, Nr]; H [4, ...], dH [3, 4, ...]."""
+        import torch
+        for t, nm in ((u, "u"), (H, "H"), (dH, "dH")):
+            _dev_f64(t, nm)
+        if u.numel() != 50 * self.Np * self.Nt * self.Nr or H.numel() * 3 != dH.numel() or H.numel() * 50 != 4 * u.numel():
+            raise ValueError("rhs_ghg: u must hold 50 fields, H 4, dH 12")
+        if out is None:
+            out = torch.empty_like(u)
+        _dev_f64(out, "out")
+        nbytes = self.ghg_workspace_bytes()
+        ws = workspace if workspace is not None else self._workspace(nbytes, u.device)
+        _check(lib().sp_rhs_ghg(self._h, u.data_ptr(), H.data_ptr(), dH.data_ptr(), out.data_ptr(), 1 if bc_outer else 0,
+                                ws.data_ptr(), ws.numel() * ws.element_size(), _stream_ptr(stream)), "sp_rhs_ghg")
+        return out
+
+    def ghg_init(self, g, stream=None):
+        """Initial data of PAPER.md:732-737 from a static metric g [10, Np, Nt, Nr]: d = gradient of g, k by (A.6),
+        H = -Gamma (A.18), dH = gradient of H.  Returns (u [50], H [4], dH [3, 4])."""
+        import torch
+        _dev_f64(g, "g")
+        shape = (self.Np, self.Nt, self.Nr)
+        u = torch.zeros((50,) + shape, dtype=torch.float64, device=g.device)
+        u[:10].copy_(g.reshape((10,) + shape))
+        u[20:].copy_(self.cartesian_gradient(u[:10], stream=stream).reshape((30,) + shape))
+        H = torch.empty((4,) + shape, dtype=torch.float64, device=g.device)
+        _check(lib().sp_ghg_init(self._h, u.data_ptr(), H.data_ptr(), _stream_ptr(stream)), "sp_ghg_init")
+        dH = self.cartesian_gradient(H, stream=stream).reshape((3, 4) + shape)
+        return u, H, dH
 
     @staticmethod
     def axpby(a, x, b, y, stream=None):

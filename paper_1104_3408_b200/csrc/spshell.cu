@@ -229,6 +229,7 @@ extern "C" sp_status sp_get_matrix(const sp_shell *s, int which, int n, int m, d
 #include "kernels_filter.cuh"
 #include "kernels_theta2.cuh"
 #include "kernels_wave.cuh"
+#include "kernels_ghg.cuh"
 
 // fork the side stream off the caller's stream / join it back (events; capture-safe; no host synchronisation)
 static bool sp_fork(const sp_shell *s, cudaStream_t st) {
@@ -751,6 +752,42 @@ extern "C" sp_status sp_rhs_first_order_wave(const sp_shell *s, const double *u,
     g_sp_launches += 1;
     k_wave_rhs<<<(unsigned)((npts + T - 1) / T), T, 0, (cudaStream_t)stream>>>(s->Nr, s->Nt, npts, s->d_sin_t, s->d_cos_t, s->d_sin_p,
                                                                               s->d_cos_p, u, dg, dudt);
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
+// ---- GHG system (Appendix A)
+extern "C" sp_status sp_ghg_workspace_bytes(const sp_shell *s, size_t *bytes) {
+    if (!s || !bytes) return SP_ERR_INVALID_ARG;
+    *bytes = (size_t)(150 + 50) * s->npts * sizeof(double);      // gradient of the 50 fields + the gradient call's own workspace
+    return SP_OK;
+}
+
+extern "C" sp_status sp_rhs_ghg(const sp_shell *s, const double *u, const double *H, const double *dH, double *dudt, int bc_outer,
+                                void *ws, size_t wsb, void *stream) {
+    if (!s || !u || !H || !dH || !dudt || dudt == u) return SP_ERR_INVALID_ARG;
+    if (!s->built) return SP_ERR_NOT_BUILT;
+    const size_t npts = s->npts;
+    if (!ws || wsb < 200 * npts * sizeof(double)) return SP_ERR_INVALID_ARG;
+    double *du = (double *)ws, *gws = du + 150 * npts;
+    sp_status e = sp_cartesian_gradient(s, u, 50, du, gws, 50 * npts * sizeof(double), stream);
+    if (e != SP_OK) return e;
+    GhgArgs A = {u, du, H, dH, dudt, npts};
+    g_sp_launches += 1;
+    k_ghg_rhs<<<(unsigned)((npts + 127) / 128), 128, 0, (cudaStream_t)stream>>>(A);
+    if (bc_outer) {
+        const int nb = s->Nt * s->Np;
+        g_sp_launches += 1;
+        k_ghg_bc<<<(nb + 127) / 128, 128, 0, (cudaStream_t)stream>>>(u, dudt, npts, s->Nr, s->Nt, s->Np, s->d_sin_t, s->d_cos_t, s->d_sin_p,
+                                                                      s->d_cos_p);
+    }
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
+extern "C" sp_status sp_ghg_init(const sp_shell *s, double *u, double *H, void *stream) {
+    if (!s || !u || !H) return SP_ERR_INVALID_ARG;
+    if (!s->built) return SP_ERR_NOT_BUILT;
+    g_sp_launches += 1;
+    k_ghg_init<<<(unsigned)((s->npts + 127) / 128), 128, 0, (cudaStream_t)stream>>>(u, H, s->npts);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
 
