@@ -36,6 +36,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--leg", default="main", choices=["main", "ghg", "ghg_rhs"],
+                    help="ghg: run only the GHG single-black-hole leg (SURVEY.md 8(f) NEXT-1) and print its JSON")
     ap.add_argument("--no-graph", action="store_true", help="time eager launches instead of replayed CUDA graphs of the step")
     return ap.parse_args()
 
@@ -470,6 +472,76 @@ class GpuWorkload:
         return ms, hu.numel() * 8, (hdu.numel() + hfu.numel()) * 8
 
 
+def ghg_e1_leg(evolve=True):
+    """The paper's own application (Sec. 4.1, Tab. 4): 1000 RK4 steps of the GHG system for the
+    Kerr-Schild black hole on the shell R10 = [1.8, 11.8] at the paper's three grids, Yn filter with n_f = 4 after every
+    step, lambda = 4, freezing outer boundary; each RK4 step is one replayed CUDA graph.  Reports the wall time of the 1000
+    steps next to the paper's GTX580 / one-core i7-870 times (context: other hardware) and rhs(g_tt) on the innermost sphere
+    at t = 0 and at the end (Fig. 2: the run must settle, not grow)."""
+    import torch
+    import synth
+    from paper_1104_3408_b200 import Shell
+    from paper_1104_3408_b200.ghg import GhgRK4
+    from paper_1104_3408_b200.wave import wave_dt
+    out = {"what": "1000 RK4 steps, 50-field GHG system, single Kerr-Schild black hole, shell [1.8, 11.8], Yn filter n_f = 4, lambda = 4",
+           "paper_tab4_seconds": {"25x9x18": {"gtx580": 16, "i7_870_one_core": 165}, "37x15x30": {"gtx580": 49, "i7_870_one_core": 823},
+                                  "49x21x42": {"gtx580": 133, "i7_870_one_core": 2903}}, "grids": {}}
+    rmin, rmax = 1.8, 11.8
+    for Nr, Nt, Np in (((25, 9, 18), (37, 15, 30), (49, 21, 42)) if evolve else ()):
+        sh = Shell(Nr, Nt, Np, rmin, rmax, Nt - 1 - 4)
+        g = torch.from_numpy(synth.kerr_schild_metric(Nr, Nt, Np, rmin, rmax)).cuda()
+        u, H, dH = sh.ghg_init(g)
+        rk = GhgRK4(sh, H, dH)
+        r_init = rk.rhs(u)
+        n0, m0 = float(r_init[0, :, :, 0].abs().max()), float(r_init.abs().max())
+        dt = wave_dt(Nr, Nt, Np, rmin, rmax, lam=4.0)
+        keep = u.clone()
+        rk.evolve(u, dt, 3, graph=True)
+        u.copy_(keep)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        rk.evolve(u, dt, 1000, graph=True)
+        e1.record()
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        r_end = rk.rhs(u)
+        n1, m1 = float(r_end[0, :, :, 0].abs().max()), float(r_end.abs().max())
+        out["grids"][f"{Nr}x{Nt}x{Np}"] = {"seconds_1000_steps": e0.elapsed_time(e1) * 1e-3, "wall_seconds": wall, "dt": dt,
+                                           "t_end": 1000 * dt, "rhs_gtt_inner_sphere_t0": n0, "rhs_gtt_inner_sphere_end": n1,
+                                           "rhs_all_fields_t0": m0, "rhs_all_fields_end": m1,
+                                           "max_drift_of_state": float((u - keep).abs().max())}
+    # the right-hand side alone on the config-3 grid (152 064 points x 50 fields): gradient + pointwise algebra + boundary
+    Nr, Nt, Np = 33, 48, 96
+    sh = Shell(Nr, Nt, Np, 1.8, 20.0, 43)
+    g = torch.from_numpy(synth.kerr_schild_metric(Nr, Nt, Np, 1.8, 20.0)).cuda()
+    u, H, dH = sh.ghg_init(g)
+    rk = GhgRK4(sh, H, dH)
+    du = torch.empty((3, 50, Np, Nt, Nr), dtype=torch.float64, device="cuda")
+    ws = torch.empty(50 * Np * Nt * Nr, dtype=torch.float64, device="cuda")
+
+    def timeit(fn, reps=50):
+        for _ in range(5):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+    t_rhs = timeit(lambda: rk.rhs(u))
+    t_grad = timeit(lambda: sh.cartesian_gradient(u, out=du, workspace=ws))
+    npts = Nr * Nt * Np
+    out["rhs_on_config3_grid"] = {"rhs_total_ms": t_rhs, "gradient_ms": t_grad, "pointwise_and_boundary_ms": t_rhs - t_grad,
+                                  "pointwise_bytes": 266 * 8 * npts,
+                                  "pointwise_GBs": 266 * 8 * npts / ((t_rhs - t_grad) * 1e-3) * 1e-9,
+                                  "note": "pointwise kernel: 216 doubles read + 50 written per point (HBM-bound by design)"}
+    return out
+
+
 def roofline_for(cfg, stages_ms, units, peak_tf, hbm_gbs, hbm_src):
     fl = flops_per_unit(cfg)
     table = {}
@@ -651,6 +723,10 @@ def run_ours(args):
                 others["config5"]["rk4_steps_per_s"] = 200.0 / (min(msw, msg) * 1e-3)
             wl = w2
         line["other_configs"] = others
+        try:
+            line["ghg_single_black_hole"] = ghg_e1_leg()
+        except Exception as ex:                       # the widened path must never cost the headline line
+            line["ghg_single_black_hole"] = {"error": repr(ex)}
     if not args.no_cpu_baseline and world == 1:
         threads = os.cpu_count() or 1
         pu, wall, desc = oracle_sample(cfg, synth.make_state(cfg), threads)
@@ -679,6 +755,9 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.leg in ("ghg", "ghg_rhs"):           # ghg_rhs: only the right-hand side on the config-3 grid (for profiling)
+        print(json.dumps({"leg": "ghg_single_black_hole", **ghg_e1_leg(evolve=args.leg == "ghg")}))
+        return 0
     return run_ours(args)
 
 
