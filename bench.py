@@ -36,8 +36,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--leg", default="main", choices=["main", "ghg", "ghg_rhs"],
+    ap.add_argument("--leg", default="main", choices=["main", "ghg", "ghg_rhs", "filters"],
                     help="ghg: run only the GHG single-black-hole leg (SURVEY.md 8(f) NEXT-1) and print its JSON")
+    ap.add_argument("--t-end", type=float, default=20000.0, help="--leg filters: evolve every filter variant to this time")
     ap.add_argument("--no-graph", action="store_true", help="time eager launches instead of replayed CUDA graphs of the step")
     return ap.parse_args()
 
@@ -542,6 +543,38 @@ def ghg_e1_leg(evolve=True):
     return out
 
 
+def filter_comparison_leg(t_end, every=5000.0):
+    """PAPER.md Sec. 4.1, Fig. 5-6 (SURVEY.md experiment E3, NEXT-2): the single black hole on 25 x 9 x 18 evolved with the
+    scalar Y-filter, the graded Yg-filter (eq. 59) and the tensor Yn-filter; max |rhs(g_tt)| on the innermost sphere is
+    sampled every `every` in t.  The paper: Y fails by t ~ 7 000, Yg by ~ 70 000, Yn runs beyond 200 000."""
+    import torch
+    import synth
+    from paper_1104_3408_b200 import Shell
+    from paper_1104_3408_b200.ghg import GhgRK4
+    from paper_1104_3408_b200.wave import wave_dt
+    Nr, Nt, Np, rmin, rmax = 25, 9, 18, 1.8, 11.8
+    dt = wave_dt(Nr, Nt, Np, rmin, rmax, lam=4.0)
+    out = {"what": "single black hole, 25x9x18, shell [1.8, 11.8], n_f = 4, lambda = 4: max|rhs(g_tt)| on the inner sphere vs t",
+           "paper": "Y fails by t ~ 7e3, Yg by ~ 7e4, Yn lasts beyond 2e5 (PAPER.md:523-543)", "dt": dt, "runs": {}}
+    for mode in ("Y", "Yg", "Yn"):
+        sh = Shell(Nr, Nt, Np, rmin, rmax, Nt - 1 - 4)
+        g = torch.from_numpy(synth.kerr_schild_metric(Nr, Nt, Np, rmin, rmax)).cuda()
+        u, H, dH = sh.ghg_init(g)
+        rk = GhgRK4(sh, H, dH, filter=mode)
+        chunk = max(1, int(every / dt))
+        t, rows, t0, failed_at = 0.0, [], time.perf_counter(), None
+        while t < t_end:
+            rk.evolve(u, dt, chunk, graph=True)
+            t += chunk * dt
+            n = float(rk.rhs(u)[0, :, :, 0].abs().max())
+            rows.append([round(t, 1), n])
+            if not (n == n) or n > 1.0:
+                failed_at = t
+                break
+        out["runs"][mode] = {"samples_t_rhs": rows, "failed_by_t": failed_at, "reached_t": t, "wall_seconds": time.perf_counter() - t0}
+    return out
+
+
 def roofline_for(cfg, stages_ms, units, peak_tf, hbm_gbs, hbm_src):
     fl = flops_per_unit(cfg)
     table = {}
@@ -755,6 +788,9 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.leg == "filters":
+        print(json.dumps({"leg": "filter_comparison", **filter_comparison_leg(args.t_end)}))
+        return 0
     if args.leg in ("ghg", "ghg_rhs"):           # ghg_rhs: only the right-hand side on the config-3 grid (for profiling)
         print(json.dumps({"leg": "ghg_single_black_hole", **ghg_e1_leg(evolve=args.leg == "ghg")}))
         return 0

@@ -102,6 +102,7 @@ class Shell:
         self._h = C.c_void_p()
         _check(lib().sp_shell_create(Nr, Ntheta, Nphi, float(r_in), float(r_out), L, C.byref(self._h)), "sp_shell_create")
         self.Nr, self.Nt, self.Np, self.L = Nr, Ntheta, Nphi, L
+        self.r_in, self.r_out = float(r_in), float(r_out)
         self.npts = Nr * Ntheta * Nphi
         self._ws = None
         if build:

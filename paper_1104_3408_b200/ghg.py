@@ -15,18 +15,46 @@ def ghg_tensors():
     ]
 
 
+def spatial_degree():
+    """d(u^mu) of PAPER.md:441: the number of spatial indices of each of the 50 Cartesian components."""
+    ab = [0, 1, 1, 1, 2, 2, 2, 2, 2, 2]
+    return ab + ab + [1 + q for _ in range(3) for q in ab]
+
+
+def scalar_tensors(fields):
+    return [{"name": f"u{q}", "rank": 0, "dims": (), "sym": (-1, -1), "fields": [q]} for q in fields]
+
+
 class GhgRK4:
-    def __init__(self, shell, H, dH, bc_outer=True):
+    """filter: "Yn" (spin-weighted tensor filter, the method of the paper), "Y" (every component filtered as a scalar with
+    the same L), "Yg" (graded scalar filter, eq. 59: component mu keeps l <= L + d(u^mu); the same kernels with the matrix
+    tables of four shells of kept degree L .. L+3) -- the three filters compared in PAPER.md Sec. 3.5 / 4.1 (Fig. 5-6)."""
+
+    def __init__(self, shell, H, dH, bc_outer=True, filter="Yn"):
         import torch
+        from .binding import Shell
         self.sh, self.H, self.dH, self.bc = shell, H, dH, bc_outer
-        self.tensors = ghg_tensors()
-        self.descs = shell.make_descs(self.tensors)
+        self.filter_mode = filter
+        if filter == "Yn":
+            self.passes = [(shell, ghg_tensors())]
+        elif filter == "Y":
+            self.passes = [(shell, scalar_tensors(range(50)))]
+        elif filter == "Yg":
+            deg = spatial_degree()
+            self.passes = []
+            for dgr in range(4):
+                L = min(shell.L + dgr, shell.Nt - 1)
+                shd = shell if dgr == 0 else Shell(shell.Nr, shell.Nt, shell.Np, shell.r_in, shell.r_out, L)
+                self.passes.append((shd, scalar_tensors([q for q in range(50) if deg[q] == dgr])))
+        else:
+            raise ValueError("filter must be 'Yn', 'Y' or 'Yg'")
+        self.passes = [(shd, t, shd.make_descs(t)) for shd, t in self.passes]
         dev = torch.device("cuda")
         shape = (50, shell.Np, shell.Nt, shell.Nr)
         self.k = torch.empty(shape, dtype=torch.float64, device=dev)
         self.acc = torch.empty(shape, dtype=torch.float64, device=dev)
         self.stage = torch.empty(shape, dtype=torch.float64, device=dev)
-        _, f, _ = shell.workspace_bytes(50)
+        f = max(shd.workspace_bytes(50)[1] for shd, _, _ in self.passes)
         self.ws_r = torch.empty(shell.ghg_workspace_bytes() // 8, dtype=torch.float64, device=dev)
         self.ws_f = torch.empty(f // 8, dtype=torch.float64, device=dev)
         self._graph, self._graph_key = None, None
@@ -35,7 +63,8 @@ class GhgRK4:
         return self.sh.rhs_ghg(v, self.H, self.dH, out=self.k if out is None else out, bc_outer=self.bc, workspace=self.ws_r)
 
     def filter(self, v):
-        self.sh.tensor_filter(v, self.tensors, out=v, workspace=self.ws_f, descs=self.descs)
+        for shd, tensors, descs in self.passes:      # fields outside a pass are left as they are
+            shd.tensor_filter(v, tensors, out=v, workspace=self.ws_f, descs=descs)
 
     def _step(self, u, dt):
         st = self.sh.rk4_stage
