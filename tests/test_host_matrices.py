@@ -59,3 +59,13 @@ def test_host_matrices_match_oracle(cfg):
         for m in range(0, L + 1):
             worst = max(worst, np.max(np.abs(sh.get_matrix(5, n, m) - oracle.filter_matrix(Nt, L, n, m))))
     assert worst < 1e-13, worst
+
+
+def test_ghg_spatial_degree_and_layout():
+    """Host logic of the GHG driver: d(u^mu) of PAPER.md:441 (g_tt 0, g_tx 1, g_xx 2; d_iab one more) and the tensor layout."""
+    from paper_1104_3408_b200.ghg import ghg_tensors, spatial_degree
+    d = spatial_degree()
+    assert len(d) == 50 and d[0] == 0 and d[1] == 1 and d[4] == 2 and d[20] == 1 and d[21] == 2 and d[24] == 3
+    assert [d.count(q) for q in range(4)] == [2, 9, 21, 18]
+    t = ghg_tensors()
+    assert sorted(sum((x["fields"] for x in t), [])) == list(range(50))
