@@ -36,7 +36,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--leg", default="main", choices=["main", "ghg", "ghg_rhs", "filters"],
+    ap.add_argument("--leg", default="main", choices=["main", "ghg", "ghg_rhs", "filters", "fft"],
                     help="ghg: run only the GHG single-black-hole leg (SURVEY.md 8(f) NEXT-1) and print its JSON")
     ap.add_argument("--t-end", type=float, default=20000.0, help="--leg filters: evolve every filter variant to this time")
     ap.add_argument("--no-graph", action="store_true", help="time eager launches instead of replayed CUDA graphs of the step")
@@ -575,6 +575,56 @@ def filter_comparison_leg(t_end, every=5000.0):
     return out
 
 
+def fft_comparison_leg():
+    """PAPER.md Sec. 4.2, Fig. 9: one-directional periodic derivative of n1 x (20*20*54) values, by matrix
+    multiplication and by FFT, against n1.  A measurement with library calls on both sides (cuBLAS DGEMM through torch.matmul,
+    cuFFT through torch.fft, each in its best layout), plus this library's own d/dphi stage (GEMM + chain-rule epilogue, two
+    outputs) on a shell with Nphi = n1 and about the same number of columns."""
+    import torch
+    from paper_1104_3408_b200 import Shell
+    cols = 20 * 20 * 54
+    out = {"what": "derivative along one periodic direction of an n1 x 21600 array, FP64: time in microseconds",
+           "paper": "matmul competitive with CUFFT up to n1 ~ 100 on GTX580/M2070 (PAPER.md:563-567, Fig. 9)", "rows": []}
+
+    def timeit(fn, reps=50):
+        for _ in range(5):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps * 1e3
+    for n1 in (16, 24, 32, 48, 64, 96, 128, 160, 192, 256):
+        x = torch.randn(n1, cols, dtype=torch.float64, device="cuda")          # GEMM layout: D [n1 x n1] @ X [n1 x cols]
+        xt = x.t().contiguous()                                                   # FFT layout: cols transforms of length n1, contiguous
+        D = torch.randn(n1, n1, dtype=torch.float64, device="cuda")
+        ik = (1j * torch.fft.rfftfreq(n1, 1.0 / n1).to("cuda")).to(torch.complex128)
+        t_mm = timeit(lambda: torch.matmul(D, x))
+        t_fft = timeit(lambda: torch.fft.irfft(torch.fft.rfft(xt, dim=1) * ik, n=n1, dim=1))
+        row = {"n1": n1, "cublas_dgemm_us": t_mm, "cufft_rfft_mul_irfft_us": t_fft}
+        Nt = n1 // 2
+        if Nt >= 4:
+            Nr = 15
+            nf = max(1, round(cols / (Nr * Nt)))
+            sh = Shell(Nr, Nt, n1, 1.0, 2.0, Nt - 1)
+            u = torch.randn(nf, n1, Nt, Nr, dtype=torch.float64, device="cuda")
+            du = torch.empty((3, nf, n1, Nt, Nr), dtype=torch.float64, device="cuda")
+            ws = torch.empty(nf * n1 * Nt * Nr, dtype=torch.float64, device="cuda")
+            sh.profile(True)
+            ts = []
+            for _ in range(7):
+                sh.cartesian_gradient(u, out=du, workspace=ws)
+                ts.append(sh.profile_read()["grad_dphi"])
+            sh.profile(False)
+            row["ours_dphi_with_chain_rule_us"] = sorted(ts)[len(ts) // 2] * 1e3
+            row["ours_columns"] = nf * Nr * Nt
+        out["rows"].append(row)
+    return out
+
+
 def roofline_for(cfg, stages_ms, units, peak_tf, hbm_gbs, hbm_src):
     fl = flops_per_unit(cfg)
     table = {}
@@ -788,6 +838,9 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.leg == "fft":
+        print(json.dumps({"leg": "fft_comparison", **fft_comparison_leg()}))
+        return 0
     if args.leg == "filters":
         print(json.dumps({"leg": "filter_comparison", **filter_comparison_leg(args.t_end)}))
         return 0
