@@ -12,6 +12,7 @@
 
 #include <cstdint>
 #include <cstdlib>
+#include <algorithm>
 
 #define PG_NCOL 64
 #define PG_KC 16
@@ -40,6 +41,14 @@ __global__ void __launch_bounds__(NC * 8)
 k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const double *__restrict__ B, long sBk, long sBb,
            double *__restrict__ C, long sCm, long sCb, int ncols, PhiGradEpi ge) {
     extern __shared__ __align__(16) double sm[];
+    if (gridDim.z > 1) {                                // row blocks: this CTA owns rows [r0, r0 + Mpad / gridDim.z)
+        Mpad /= gridDim.z;
+        const int r0 = blockIdx.z * Mpad;
+        M = min(M - r0, Mpad);
+        A += (long)r0 * lda;
+        C += (long)r0 * sCm;
+        if (EPI_GRAD) { ge.Y += (long)r0 * sCm; ge.sin_p += r0; ge.cos_p += r0; }
+    }
     // plain products: K chunks of 16, 3 stages; gradient variant (which also holds the W tile): chunks of 8, 4 stages
     constexpr int KC = EPI_GRAD ? 8 : 16, STG = EPI_GRAD ? 4 : 3, PA = KC + 4;
     constexpr int PG_PB = NC + 4, PG_PW = NC + 8, NG = NC / 16, HC = NC / 2;
@@ -191,13 +200,21 @@ static sp_status launch_phi_gemm(const double *A, int lda, int M, const PhiTilin
     if (((uintptr_t)B | (uintptr_t)C) & 15) return SP_ERR_UNSUPPORTED;
     if (tl.mgroups > 4) return SP_ERR_UNSUPPORTED;
     const int NC = phi_ncol(ncols, nbatch);
-    dim3 grid((ncols + NC - 1) / NC, nbatch), block(tl.mgroups * (NC / 16) * 32);
+    // row blocks: plain products with two warp rows and many column tiles run as two CTAs of half the rows (measured at config 4:
+    // analysis -9 %, synthesis -4 %; no gain for the gradient variant or at config 3).  SP_PHI_MSPLIT overrides (experiments).
+    static const int msplit_env = [] { const char *e = getenv("SP_PHI_MSPLIT"); return e ? atoi(e) : -1; }();
+    const long ctas = (long)((ncols + NC - 1) / NC) * nbatch;
+    int zs = (!ge && tl.mgroups == 2 && ctas >= 8L * g_sp_num_sms) ? 2 : 1;
+    if (msplit_env >= 1) zs = (tl.mgroups % msplit_env == 0) ? msplit_env : 1;
+    PhiTiling tz = tl;
+    tz.mgroups = tl.mgroups / zs; tz.Mpad = tl.Mpad / zs;
+    dim3 grid((ncols + NC - 1) / NC, nbatch, zs), block(tz.mgroups * (NC / 16) * 32);
 #define SP_PG(MTV, EPIV, SM, GE)                                                                                              \
     if (NC == 32) k_phi_gemm<MTV, EPIV, 32><<<grid, block, SM, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, GE); \
     else k_phi_gemm<MTV, EPIV, 64><<<grid, block, SM, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, GE);
     if (ge) {
         if ((ge->sYb & 1) || ((uintptr_t)ge->Y & 15)) return SP_ERR_UNSUPPORTED;
-        const size_t sm = phi_smem_bytes(tl, M, NC);
+        const size_t sm = phi_smem_bytes(tz, std::min(M, tz.Mpad), NC);
         if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;
         switch (tl.MT) {
             case 4: SP_PG(4, true, sm, *ge) break;
@@ -206,7 +223,7 @@ static sp_status launch_phi_gemm(const double *A, int lda, int M, const PhiTilin
         }
         return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
     }
-    const size_t sm = phi_smem_bytes(tl, 0, NC);
+    const size_t sm = phi_smem_bytes(tz, 0, NC);
     PhiGradEpi none = {};
     switch (tl.MT) {
         case 4: SP_PG(4, false, sm, none) break;
