@@ -622,6 +622,14 @@ def fft_comparison_leg():
             row["ours_dphi_with_chain_rule_us"] = sorted(ts)[len(ts) // 2] * 1e3
             row["ours_columns"] = nf * Nr * Nt
         out["rows"].append(row)
+    # the d/dphi product of config 3 in its own layout: 50 fields x [96 x 96] @ [96 x 1584] (K stride 1584), cuBLAS batched
+    X = torch.randn(50, 96, 1584, dtype=torch.float64, device="cuda")
+    D = torch.randn(96, 96, dtype=torch.float64, device="cuda")
+    Y = torch.empty_like(X)
+    t = timeit(lambda: torch.matmul(D, X, out=Y))
+    out["config3_dphi_shape"] = {"cublas_batched_dgemm_us": t, "tflops": 2.0 * 96 * 96 * 50 * 1584 / t * 1e-6,
+                                 "note": "product only; the library's stage (grad_dphi in the main line) also applies the chain rule "
+                                         "and writes d_x and d_y (another 2 x 61 MB read and 2 x 61 MB written)"}
     return out
 
 
