@@ -27,9 +27,10 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
 // EPI_GRAD: gradient epilogue (eq. 6).  The product is d/dphi u (A = FD_{Nphi}); C holds on entry the
-// phi-independent combination W written by k_grad_rtheta2<.., SPLIT> and receives d_x u; Y receives d_y u:
+// phi-independent combination W written by k_grad_rtheta3 and receives d_x u; Y receives d_y u:
 //     c = (d_phi u)/(r sin th),   d_x = cos(ph) W - sin(ph) c,   d_y = sin(ph) W + cos(ph) c.
-// The CTA's W tile [M][64] is fetched by cp.async at kernel start into its own shared-memory tile (pitch 72).
+// Two-phase epilogue: c is parked in shared memory (the pipeline buffers are free by then), then all threads walk the tile
+// row-contiguously with coalesced 16-byte loads of W and stores of d_x, d_y.
 struct PhiGradEpi {
     double *Y; long sYb;                      // d_y output, batch stride
     const double *inv_r, *inv_sin_t, *sin_p, *cos_p;
@@ -49,12 +50,11 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
         C += (long)r0 * sCm;
         if (EPI_GRAD) { ge.Y += (long)r0 * sCm; ge.sin_p += r0; ge.cos_p += r0; }
     }
-    // plain products: K chunks of 16, 3 stages; gradient variant (which also holds the W tile): chunks of 8, 4 stages
-    constexpr int KC = EPI_GRAD ? 8 : 16, STG = EPI_GRAD ? 4 : 3, PA = KC + 4;
-    constexpr int PG_PB = NC + 4, PG_PW = NC + 8, NG = NC / 16, HC = NC / 2;
+    // K chunks of 16, 3 stages
+    constexpr int KC = 16, STG = 3, PA = KC + 4;
+    constexpr int PG_PB = NC + 4, PG_PC = NC + 2, NG = NC / 16, HC = NC / 2;
     const int stageA = Mpad * PA, stageB = KC * PG_PB;
     double *As = sm, *Bs = sm + STG * stageA;
-    double *Ws = Bs + STG * stageB;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp / NG, ng = warp % NG;
     const int c0 = blockIdx.x * NC;
@@ -87,13 +87,6 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
 #pragma unroll
         for (int b = 0; b < 2; b++) acc[a][b][0] = acc[a][b][1] = 0.0;
 
-    if (EPI_GRAD) {      // oldest cp.async group: complete long before the epilogue
-        for (int q = tid; q < M * HC; q += blockDim.x) {
-            const int r = q / HC, h = q % HC;
-            if (2 * h < colsleft) cp_async16(Ws + r * PG_PW + 2 * h, Cb + (long)r * sCm + 2 * h);
-        }
-        cp_async_commit();
-    }
 #pragma unroll
     for (int s = 0; s < STG - 1; s++) {
         if (s < nchunks) load_chunk(s, s);
@@ -133,32 +126,54 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
             }
         }
     } else {
+        // two phases.  (1) every lane scales its accumulators to c = d_phi u /(r sin th) and parks them in shared memory (the
+        // pipeline buffers are free now) as an [M][NC] tile.  (2) all threads walk the tile row-contiguously: coalesced 16-byte
+        // loads of W, coalesced stores of d_x and d_y, several independent loads in flight per thread.
         cp_async_wait<0>();
-        __syncthreads();                       // W tile (copied by all threads) visible to all
+        __syncthreads();
+        double *cs = sm;
         double *Yb = ge.Y + (long)blockIdx.y * ge.sYb + c0;
-        double f[2][2];                        // 1/(r sin th) of the lane's four columns
+        {
+            double f[2][2];                    // 1/(r sin th) of the lane's four columns
 #pragma unroll
-        for (int b = 0; b < 2; b++)
+            for (int b = 0; b < 2; b++)
 #pragma unroll
-            for (int e = 0; e < 2; e++) {
-                const int c = c0 + ng * 16 + b * 8 + 2 * t + e;        // flat (k, i) column: c = k + Nr i
-                const int i = c / ge.Nr, k = c - i * ge.Nr;
-                f[b][e] = (c < ncols) ? __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i) : 0.0;
+                for (int e = 0; e < 2; e++) {
+                    const int c = c0 + ng * 16 + b * 8 + 2 * t + e;        // flat (k, i) column: c = k + Nr i
+                    const int i = c / ge.Nr, k = c - i * ge.Nr;
+                    f[b][e] = (c < ncols) ? __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i) : 0.0;
+                }
+#pragma unroll
+            for (int a = 0; a < MT; a++) {
+                const int row = (mg * MT + a) * 8 + g;                       // longitude j
+                if (row >= M) continue;
+#pragma unroll
+                for (int b = 0; b < 2; b++)
+                    *reinterpret_cast<double2 *>(cs + row * PG_PC + ng * 16 + b * 8 + 2 * t) =
+                        make_double2(acc[a][b][0] * f[b][0], acc[a][b][1] * f[b][1]);
+            }
+        }
+        __syncthreads();
+        const int npair = min(NC, colsleft) >> 1;
+        constexpr int UNR = 4;
+        for (int q0 = tid; q0 < M * HC; q0 += UNR * blockDim.x) {
+            double2 w[UNR];
+            int row[UNR], cp2[UNR];
+            bool ok[UNR];
+#pragma unroll
+            for (int z = 0; z < UNR; z++) {
+                const int q = q0 + z * blockDim.x;
+                row[z] = q / HC; cp2[z] = q % HC;
+                ok[z] = q < M * HC && cp2[z] < npair;
+                if (ok[z]) w[z] = *reinterpret_cast<const double2 *>(Cb + (long)row[z] * sCm + 2 * cp2[z]);
             }
 #pragma unroll
-        for (int a = 0; a < MT; a++) {
-            const int row = (mg * MT + a) * 8 + g;                       // longitude j
-            if (row >= M) continue;
-            const double sp = __ldg(ge.sin_p + row), cp = __ldg(ge.cos_p + row);
-#pragma unroll
-            for (int b = 0; b < 2; b++) {
-                const int col = ng * 16 + b * 8 + 2 * t;
-                if (col < colsleft) {
-                    const double2 w = *reinterpret_cast<const double2 *>(Ws + row * PG_PW + col);
-                    const double ca = acc[a][b][0] * f[b][0], cb = acc[a][b][1] * f[b][1];
-                    *reinterpret_cast<double2 *>(Cb + (long)row * sCm + col) = make_double2(cp * w.x - sp * ca, cp * w.y - sp * cb);
-                    *reinterpret_cast<double2 *>(Yb + (long)row * sCm + col) = make_double2(sp * w.x + cp * ca, sp * w.y + cp * cb);
-                }
+            for (int z = 0; z < UNR; z++) {
+                if (!ok[z]) continue;
+                const double2 c = *reinterpret_cast<const double2 *>(cs + row[z] * PG_PC + 2 * cp2[z]);
+                const double sp = __ldg(ge.sin_p + row[z]), cp = __ldg(ge.cos_p + row[z]);
+                *reinterpret_cast<double2 *>(Cb + (long)row[z] * sCm + 2 * cp2[z]) = make_double2(cp * w[z].x - sp * c.x, cp * w[z].y - sp * c.y);
+                *reinterpret_cast<double2 *>(Yb + (long)row[z] * sCm + 2 * cp2[z]) = make_double2(sp * w[z].x + cp * c.x, sp * w[z].y + cp * c.y);
             }
         }
     }
@@ -179,8 +194,10 @@ static inline PhiTiling phi_tiling(int M) {
     return best;
 }
 static inline size_t phi_smem_bytes(const PhiTiling &tl, int Mgrad = 0, int NC = PG_NCOL) {
-    const int KC = Mgrad ? 8 : 16, STG = Mgrad ? 4 : 3, PA = KC + 4;
-    return ((size_t)STG * ((size_t)tl.Mpad * PA + KC * (NC + 4)) + (size_t)Mgrad * (NC + 8)) * sizeof(double);
+    const int KC = 16, STG = 3, PA = KC + 4;
+    const size_t pipe = (size_t)STG * ((size_t)tl.Mpad * PA + KC * (NC + 4)) * sizeof(double);
+    const size_t tile = (size_t)Mgrad * (NC + 2) * sizeof(double);      // the gradient epilogue's tile reuses the pipeline buffers
+    return pipe > tile ? pipe : tile;
 }
 // column tile width: 64, or 32 when 64-wide tiles would give fewer than 2 CTAs per SM (small states: more, smaller CTAs keep
 // every SM busy and let several CTAs per SM overlap their load, product and store phases).  SP_PHI_NC overrides (experiments).
@@ -200,11 +217,11 @@ static sp_status launch_phi_gemm(const double *A, int lda, int M, const PhiTilin
     if (((uintptr_t)B | (uintptr_t)C) & 15) return SP_ERR_UNSUPPORTED;
     if (tl.mgroups > 4) return SP_ERR_UNSUPPORTED;
     const int NC = phi_ncol(ncols, nbatch);
-    // row blocks: plain products with two warp rows and many column tiles run as two CTAs of half the rows (measured at config 4:
-    // analysis -9 %, synthesis -4 %; no gain for the gradient variant or at config 3).  SP_PHI_MSPLIT overrides (experiments).
+    // row blocks: products with two warp rows and many column tiles run as two CTAs of half the rows (measured: config 4
+    // analysis -9 %, synthesis -4 %; config 3 d/dphi with the chain rule -7 %).  SP_PHI_MSPLIT overrides (experiments).
     static const int msplit_env = [] { const char *e = getenv("SP_PHI_MSPLIT"); return e ? atoi(e) : -1; }();
     const long ctas = (long)((ncols + NC - 1) / NC) * nbatch;
-    int zs = (!ge && tl.mgroups == 2 && ctas >= 8L * g_sp_num_sms) ? 2 : 1;
+    int zs = (tl.mgroups == 2 && ctas >= 8L * g_sp_num_sms) ? 2 : 1;
     if (msplit_env >= 1) zs = (tl.mgroups % msplit_env == 0) ? msplit_env : 1;
     PhiTiling tz = tl;
     tz.mgroups = tl.mgroups / zs; tz.Mpad = tl.Mpad / zs;
