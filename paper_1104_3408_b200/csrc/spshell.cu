@@ -343,13 +343,19 @@ sp_status sp_configure_kernels(sp_shell *s) {
                 if (s->grad_smem[nb - 1] > 227 * 1024) continue;
                 int occ = 0;
                 const int smb = (int)s->grad_smem[nb - 1];
-#define SP_G3(KT_, NB_)                                                                                             \
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, smb));      \
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));   \
-    SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grad_rtheta3<KT_, NB_>, thr, smb));
+#define SP_G3P(KT_, NB_, PU_)                                                                                            \
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_, PU_>, cudaFuncAttributeMaxDynamicSharedMemorySize, smb));      \
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_, PU_>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));   \
+    SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grad_rtheta3<KT_, NB_, PU_>, thr, smb));
+#define SP_G3(KT_, NB_)                                                                      \
+    if (KT_ == 5 && s->PU == 44) { SP_G3P(KT_, NB_, 44) }                                    \
+    else if (KT_ == 3 && s->PU == 28) { SP_G3P(KT_, NB_, 28) }                               \
+    else if (KT_ == 3 && s->PU == 76) { SP_G3P(KT_, NB_, 76) }                               \
+    else { SP_G3P(KT_, NB_, 0) }
                 if (KT == 3) { if (nb == 1) { SP_G3(3, 1) } else { SP_G3(3, 2) } }
                 else { if (nb == 1) { SP_G3(5, 1) } else { SP_G3(5, 2) } }
 #undef SP_G3
+#undef SP_G3P
                 s->grad3_ctas[nb - 1] = occ;
             }
         }
@@ -478,8 +484,14 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
             const int nb = (s->grad3_ctas[1] > 0 && p.nitems >= 3 * s->num_sms * s->grad3_ctas[1]) ? 2 : 1;
             const int ncta = std::min(p.nitems, s->num_sms * s->grad3_ctas[nb - 1]);
             const size_t smb = s->grad_smem[nb - 1];
-            if (KT == 3) { if (nb == 2) k_grad_rtheta3<3, 2><<<ncta, nthr, smb, st>>>(p); else k_grad_rtheta3<3, 1><<<ncta, nthr, smb, st>>>(p); }
-            else { if (nb == 2) k_grad_rtheta3<5, 2><<<ncta, nthr, smb, st>>>(p); else k_grad_rtheta3<5, 1><<<ncta, nthr, smb, st>>>(p); }
+#define SP_G3L(KT_, NB_)                                                                               \
+    if (KT_ == 5 && s->PU == 44) k_grad_rtheta3<KT_, NB_, 44><<<ncta, nthr, smb, st>>>(p);             \
+    else if (KT_ == 3 && s->PU == 28) k_grad_rtheta3<KT_, NB_, 28><<<ncta, nthr, smb, st>>>(p);        \
+    else if (KT_ == 3 && s->PU == 76) k_grad_rtheta3<KT_, NB_, 76><<<ncta, nthr, smb, st>>>(p);        \
+    else k_grad_rtheta3<KT_, NB_, 0><<<ncta, nthr, smb, st>>>(p);
+            if (KT == 3) { if (nb == 2) { SP_G3L(3, 2) } else { SP_G3L(3, 1) } }
+            else { if (nb == 2) { SP_G3L(5, 2) } else { SP_G3L(5, 1) } }
+#undef SP_G3L
             (void)ntasks;
         } else {
 #define SPLITV true
