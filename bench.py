@@ -36,7 +36,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--leg", default="main", choices=["main", "ghg", "ghg_rhs", "filters", "fft"],
+    ap.add_argument("--leg", default="main", choices=["main", "ghg", "ghg_rhs", "filters", "fft", "convergence"],
                     help="ghg: run only the GHG single-black-hole leg (SURVEY.md 8(f) NEXT-1) and print its JSON")
     ap.add_argument("--t-end", type=float, default=20000.0, help="--leg filters: evolve every filter variant to this time")
     ap.add_argument("--no-graph", action="store_true", help="time eager launches instead of replayed CUDA graphs of the step")
@@ -575,6 +575,41 @@ def filter_comparison_leg(t_end, every=5000.0):
     return out
 
 
+def convergence_leg(t_end=1000.0):
+    """PAPER.md Sec. 4.1, Fig. 2: the single black hole evolved to t = 1000 at Ntheta x Nphi = 9 x 18 and Nr = 13 ... 37;
+    max |rhs(g_tt)| on the innermost sphere against t.  The paper: exponential convergence with Nr, the oscillation dies out
+    and the runs settle; round-off (1e-12 ... 1e-13) is reached at Nr ~ 37-40."""
+    import torch
+    import synth
+    from paper_1104_3408_b200 import Shell
+    from paper_1104_3408_b200.ghg import GhgRK4
+    from paper_1104_3408_b200.wave import wave_dt
+    Nt, Np, rmin, rmax = 9, 18, 1.8, 11.8
+    out = {"what": "single black hole, Nr x 9 x 18, shell [1.8, 11.8], Yn filter n_f = 4, lambda = 4: max|rhs(g_tt)| on the inner sphere",
+           "paper": "Fig. 2 (PAPER.md:487-505): exponential convergence with Nr; round-off 1e-12..1e-13 near Nr = 37-40", "runs": {}}
+    for Nr in (13, 17, 21, 25, 29, 33, 37):
+        sh = Shell(Nr, Nt, Np, rmin, rmax, Nt - 1 - 4)
+        g = torch.from_numpy(synth.kerr_schild_metric(Nr, Nt, Np, rmin, rmax)).cuda()
+        u, H, dH = sh.ghg_init(g)
+        rk = GhgRK4(sh, H, dH)
+        dt = wave_dt(Nr, Nt, Np, rmin, rmax, lam=4.0)
+        rows, t = [], 0.0
+        chunk = max(1, int(round(50.0 / dt)))
+        peak = 0.0
+        while t < t_end:
+            # the oscillation: sample the maximum over the chunk's last 20 steps rather than one phase of it
+            rk.evolve(u, dt, max(chunk - 20, 1), graph=True)
+            m = 0.0
+            for _ in range(20):
+                rk.evolve(u, dt, 1, graph=True)
+                m = max(m, float(rk.rhs(u)[0, :, :, 0].abs().max()))
+            t += (max(chunk - 20, 1) + 20) * dt
+            rows.append([round(t, 1), m])
+            peak = max(peak, m)
+        out["runs"][str(Nr)] = {"dt": dt, "samples_t_rhs": rows, "max_over_run": peak, "final": rows[-1][1]}
+    return out
+
+
 def fft_comparison_leg():
     """PAPER.md Sec. 4.2, Fig. 9: one-directional periodic derivative of n1 x (20*20*54) values, by matrix
     multiplication and by FFT, against n1.  A measurement with library calls on both sides (cuBLAS DGEMM through torch.matmul,
@@ -846,6 +881,9 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.leg == "convergence":
+        print(json.dumps({"leg": "radial_convergence", **convergence_leg()}))
+        return 0
     if args.leg == "fft":
         print(json.dumps({"leg": "fft_comparison", **fft_comparison_leg()}))
         return 0
