@@ -247,6 +247,11 @@ def test_bench_launch_configuration_two_streams():
         wl.graphs[n].replay()
     torch.cuda.synchronize()
     assert torch.equal(wl.du, du1) and torch.equal(wl.fu, fu1)
+    wl.du.zero_(); wl.fu.zero_()
+    wl.round_graph.replay()                                  # sets 0, 1 in one graph without an inner join ...
+    wl.graphs[0].replay()                                    # ... then set 0 again
+    torch.cuda.synchronize()
+    assert torch.equal(wl.du, du1) and torch.equal(wl.fu, fu1)
     u = wl.u_host
     got = wl.du.cpu().numpy()
     rng = np.random.default_rng(33)
