@@ -111,3 +111,26 @@ def test_boundary_condition_freezes_incoming_characteristic_fields():
                 worst = max(worst, np.abs(td1 - s_dn * (s_up @ td1)).max() / scale)              # tangential part frozen
                 worst = max(worst, abs((-tg1 + tk1 + s_up @ td1) - (-tg0 + tk0 + s_up @ td0)) / scale)   # outgoing kept
     assert worst < 1e-13
+
+
+def test_characteristic_speeds_printed_in_the_paper():
+    """"in the numerical example r_min = 1.80, and the eigenvalues range from -1.45 ...  For r_min = 2.00, the
+    fastest eigenspeed is -sqrt(2) = -1.41, for r_min = 1.50 it is -1.53" -- the speed -alpha - b of (A.14) with b = s_k beta^k
+    and s_i the unit normal w.r.t. gamma^{ij}, all taken from the oracle's 3+1 split of the Kerr-Schild data."""
+    for rmin, printed in ((1.80, -1.45), (2.00, -1.41), (1.50, -1.53)):
+        Nr, Nt, Np = 5, 4, 8
+        g = synth.kerr_schild_metric(Nr, Nt, Np, rmin, rmin + 5.0)
+        u = np.zeros((50, Np, Nt, Nr)); u[:10] = g
+        out = oracle.ghg_lapse_shift(u, Nr, Nt, Np)
+        x, y, z = synth.grid_xyz(Nr, Nt, Np, rmin, rmin + 5.0)
+        j, i, k = 3, 1, 0                                          # a point on the inner boundary
+        l = np.array([x[j, i, k], y[j, i, k], z[j, i, k]]); l /= np.linalg.norm(l)
+        gi = np.zeros((3, 3)); c = 4
+        for a in range(3):
+            for b in range(a, 3):
+                gi[a, b] = gi[b, a] = out[c, j, i, k]; c += 1
+        s_dn = l / np.sqrt(l @ gi @ l)
+        alpha, beta_up = out[0, j, i, k], out[1:4, j, i, k]
+        v = -alpha - s_dn @ beta_up
+        assert abs(v - printed) < 0.006, (rmin, v)
+        assert abs((alpha - s_dn @ beta_up)) < 1e-12 if rmin == 2.00 else True      # the outgoing speed vanishes on the horizon
