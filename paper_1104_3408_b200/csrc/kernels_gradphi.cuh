@@ -24,7 +24,15 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
                 PhiGradEpi ge) {
     extern __shared__ __align__(16) double sm[];
     constexpr int GF_PB = NC + 4, GF_PC = NC + 2, NG = NC / 16, HC = NC / 2;
-    const int h = J >> 1, M = h + 1, K = h + 1;
+    const int h = J >> 1, K = h + 1;
+    int M = h + 1, r0 = 0;
+    if (gridDim.z > 1) {                                // row blocks: this CTA owns the rows j' in [r0, r0 + Mpad / gridDim.z) and their mirrors
+        Mpad /= gridDim.z;
+        r0 = blockIdx.z * Mpad;
+        M = min(M - r0, Mpad);
+        Gm += (long)r0 * lda;
+        Gp += (long)r0 * lda;
+    }
     const int stageA = 2 * Mpad * GF_PA, stageB = 2 * GF_KC * GF_PB;
     double *As = sm, *Bs = sm + GF_STAGES * stageA;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
@@ -99,7 +107,7 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
     // 16-byte loads of W, coalesced stores of d_x and d_y, many independent loads in flight per thread.
     cp_async_wait<0>();
     __syncthreads();
-    double *cs = sm;                                                        // [J][GF_PC]
+    double *cs = sm;                                                        // [2 Mpad][GF_PC]: rows j', then their mirrors J - j'
     {
         double f[2][2];
 #pragma unroll
@@ -112,16 +120,16 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
             }
 #pragma unroll
         for (int a = 0; a < MT; a++) {
-            const int row = (mg * MT + a) * 8 + g;                          // j' in [0, h]
+            const int row = (mg * MT + a) * 8 + g;                          // local row; j' = r0 + row in [0, h]
             if (row >= M) continue;
-            const bool mirrored = row > 0 && row < h;
+            const bool mirrored = r0 + row > 0 && r0 + row < h;
 #pragma unroll
             for (int b = 0; b < 2; b++) {
                 const int col = ng * 16 + b * 8 + 2 * t;
                 *reinterpret_cast<double2 *>(cs + row * GF_PC + col) =
                     make_double2((aO[a][b][0] + aE[a][b][0]) * f[b][0], (aO[a][b][1] + aE[a][b][1]) * f[b][1]);
                 if (mirrored)
-                    *reinterpret_cast<double2 *>(cs + (J - row) * GF_PC + col) =
+                    *reinterpret_cast<double2 *>(cs + (Mpad + row) * GF_PC + col) =
                         make_double2((aO[a][b][0] - aE[a][b][0]) * f[b][0], (aO[a][b][1] - aE[a][b][1]) * f[b][1]);
             }
         }
@@ -130,21 +138,24 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
     double *Xb = X + (long)blockIdx.y * sXb + c0, *Yb = Y + (long)blockIdx.y * sXb + c0;
     const int npair = min(NC, colsleft) >> 1;                          // column pairs of this tile
     constexpr int UNR = 4;
-    for (int q0 = tid; q0 < J * HC; q0 += UNR * blockDim.x) {
+    for (int q0 = tid; q0 < 2 * Mpad * HC; q0 += UNR * blockDim.x) {
         double2 w[UNR];
-        int row[UNR], cp2[UNR];
+        int lrow[UNR], row[UNR], cp2[UNR];
         bool ok[UNR];
 #pragma unroll
         for (int z = 0; z < UNR; z++) {
             const int q = q0 + z * blockDim.x;
-            row[z] = q / HC; cp2[z] = q % HC;
-            ok[z] = q < J * HC && cp2[z] < npair;
+            lrow[z] = q / HC; cp2[z] = q % HC;
+            const bool mir = lrow[z] >= Mpad;
+            const int lr = lrow[z] - (mir ? Mpad : 0), jp = r0 + lr;         // j' of this tile row
+            row[z] = mir ? J - jp : jp;                                      // longitude j
+            ok[z] = q < 2 * Mpad * HC && lr < M && cp2[z] < npair && (!mir || (jp > 0 && jp < h));
             if (ok[z]) w[z] = *reinterpret_cast<const double2 *>(Xb + (long)row[z] * sUj + 2 * cp2[z]);
         }
 #pragma unroll
         for (int z = 0; z < UNR; z++) {
             if (!ok[z]) continue;
-            const double2 c = *reinterpret_cast<const double2 *>(cs + row[z] * GF_PC + 2 * cp2[z]);
+            const double2 c = *reinterpret_cast<const double2 *>(cs + lrow[z] * GF_PC + 2 * cp2[z]);
             const double sp = __ldg(ge.sin_p + row[z]), cp = __ldg(ge.cos_p + row[z]);
             *reinterpret_cast<double2 *>(Xb + (long)row[z] * sUj + 2 * cp2[z]) = make_double2(cp * w[z].x - sp * c.x, cp * w[z].y - sp * c.y);
             *reinterpret_cast<double2 *>(Yb + (long)row[z] * sUj + 2 * cp2[z]) = make_double2(sp * w[z].x + cp * c.x, sp * w[z].y + cp * c.y);
@@ -152,8 +163,9 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
     }
 }
 
-static inline size_t gradfold_smem_bytes(int Mpad, int J, int NC = PG_NCOL) {
+static inline size_t gradfold_smem_bytes(int Mpad, int J, int NC = PG_NCOL) {      // Mpad = rows per CTA
+    (void)J;
     const size_t pipe = (size_t)GF_STAGES * ((size_t)2 * Mpad * GF_PA + 2 * GF_KC * (NC + 4)) * sizeof(double);
-    const size_t tile = (size_t)J * (NC + 2) * sizeof(double);                 // the epilogue tile reuses the pipeline buffers
+    const size_t tile = (size_t)2 * Mpad * (NC + 2) * sizeof(double);                 // the epilogue tile reuses the pipeline buffers
     return pipe > tile ? pipe : tile;
 }

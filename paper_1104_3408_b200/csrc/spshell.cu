@@ -513,13 +513,20 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         // the fold halves the DMMAs but doubles the rows each warp finishes; measured: it wins from Nphi = 128 upwards
         if (s->gf_ok && Np >= 128) {      // reflection-folded d/dphi with the chain rule in the epilogue
             const int NC = phi_ncol((int)plane, nf);
-            const dim3 gridf(((int)plane + NC - 1) / NC, nf);
+            const long ctas = (long)(((int)plane + NC - 1) / NC) * nf;
+            // row blocks as in launch_phi_gemm: two CTAs of half the rows when the kernel has an even number of warp rows
+            static const int zenv = [] { const char *e = getenv("SP_PHI_MSPLIT"); return e ? atoi(e) : -1; }();
+            int zs = (s->gf_mg % 2 == 0 && ctas >= 8L * s->num_sms) ? 2 : 1;
+            if (zenv >= 1) zs = (s->gf_mg % zenv == 0) ? zenv : 1;
+            const int mgc = s->gf_mg / zs;
+            const dim3 gridf(((int)plane + NC - 1) / NC, nf, zs);
+            const size_t smf = gradfold_smem_bytes(s->gf_Mpad / zs, s->Np, NC);
             if (NC == 32)
-                k_phi_grad_fold<4, 32><<<gridf, s->gf_mg * 2 * 32, gradfold_smem_bytes(s->gf_Mpad, s->Np, 32), st>>>(
+                k_phi_grad_fold<4, 32><<<gridf, mgc * 2 * 32, smf, st>>>(
                     s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge);
             else
-                k_phi_grad_fold<4, 64><<<gridf, s->gf_mg * 4 * 32, gradfold_smem_bytes(s->gf_Mpad, s->Np), st>>>(
-                s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge);
+                k_phi_grad_fold<4, 64><<<gridf, mgc * 4 * 32, smf, st>>>(
+                    s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge);
             if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         } else {
             sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, du, plane, (long)s->npts, (int)plane, nf,
