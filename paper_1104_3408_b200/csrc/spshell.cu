@@ -514,9 +514,11 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         if (s->gf_ok && Np >= 128) {      // reflection-folded d/dphi with the chain rule in the epilogue
             const int NC = phi_ncol((int)plane, nf);
             const long ctas = (long)(((int)plane + NC - 1) / NC) * nf;
-            // row blocks as in launch_phi_gemm: two CTAs of half the rows when the kernel has an even number of warp rows
+            // row blocks as in launch_phi_gemm: two CTAs of half the rows when the kernel has an even number of warp rows and many
+            // column tiles (config 4: 1.17 -> 0.97 ms)
             static const int zenv = [] { const char *e = getenv("SP_PHI_MSPLIT"); return e ? atoi(e) : -1; }();
             int zs = (s->gf_mg % 2 == 0 && ctas >= 8L * s->num_sms) ? 2 : 1;
+            if (ctas < 4L * s->num_sms) zs = s->gf_mg;      // small states: one warp row per CTA (config 5: d/dphi 39 -> 29 us)
             if (zenv >= 1) zs = (s->gf_mg % zenv == 0) ? zenv : 1;
             const int mgc = s->gf_mg / zs;
             const dim3 gridf(((int)plane + NC - 1) / NC, nf, zs);
