@@ -413,7 +413,7 @@ class GpuWorkload:
         ff = fl["filt_analysis"] + fl["filt_theta"] + fl["filt_synthesis"]
         out = {}
         for which, f in (("gradient", fg), ("filter", ff)):
-            ms = self.time_call(which, steps)
+            ms = sorted(self.time_call(which, steps) for _ in range(3))[1]      # median of three runs
             tf = f * self.units / (ms * 1e-3) * 1e-12
             out[which] = {"ms": ms, "value": self.units / (ms * 1e-3), "algorithmic_flops_per_unit": f, "tflops": tf,
                           "frac_of_fp64_peak": tf / peak_tf}
@@ -764,8 +764,9 @@ def run_ours(args):
     e2e_ms, h2d, d2h = wl.e2e(max(4, min(args.steps, 20)))
     e2e_ms_all, e2e_units = aggregate_over_ranks(e2e_ms, wl.units, dist if world > 1 else None)
     stages = wl.stage_times()
-    serial_ms = wl.time_steps(max(10, args.steps // 4), 2, concurrent=False) / max(10, args.steps // 4)
-    eager_ms = wl.time_steps(max(10, args.steps // 4), 2) / max(10, args.steps // 4)
+    nsec = max(10, args.steps // 4)                  # secondary figures: median of three short runs each
+    serial_ms = sorted(wl.time_steps(nsec, 2, concurrent=False) / nsec for _ in range(3))[1]
+    eager_ms = sorted(wl.time_steps(nsec, 2) / nsec for _ in range(3))[1]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
