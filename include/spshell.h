@@ -24,6 +24,12 @@
  * asynchronous on the given stream (a cudaStream_t passed as void*, NULL = default stream), do not
  * synchronise, and are deterministic (no atomics): same inputs give bit-identical outputs.
  *
+ * CONCURRENCY.  A shell owns one internal side stream and two events with which independent launches of one call
+ * (cosine / sine products, real / complex theta products, tensor groups) are forked from and joined to the caller's
+ * stream; this is legal under CUDA stream capture, so hot calls can be captured into CUDA graphs.  Calls on the same
+ * shell may be issued on different streams (e.g. the gradient on one, the filter on another), but from ONE host thread
+ * at a time: the shell's events are not protected against concurrent host threads.  Different shells are independent.
+ *
  * ERRORS.  Every call returns an sp_status; nothing throws across the ABI.
  */
 #ifndef SPSHELL_H
