@@ -80,7 +80,11 @@ sp_status sp_shell_destroy(sp_shell *shell);
  * n = -3..3, m = 0..L, built by the paper's own route: the n-recursion (42)-(44) (evaluated in
  * binary128) and the SVD pseudo-inverse.  Synchronous.  Without a CUDA device the host matrices are
  * still built (sp_get_matrix then works, so the host logic can be tested) but the call returns
- * SP_ERR_CUDA and every hot call keeps returning SP_ERR_NOT_BUILT. */
+ * SP_ERR_CUDA and every hot call keeps returning SP_ERR_NOT_BUILT.
+ * SIZE LIMIT.  The gradient kernels keep an antipodal pair of (r, theta) planes of one field in one SM's shared memory:
+ * shells with 2 * Ntheta8 * (Nr8 + 4) * 8 bytes plus the tables above 227 KB (Ntheta8, Nr8 = sizes rounded up to 8; e.g.
+ * 129 x 128 x 256) return SP_ERR_UNSUPPORTED here.  The largest BASELINE grid, 65 x 96 x 192, uses 117 KB; the method
+ * itself targets n <~ 100 per direction. */
 sp_status sp_build_matrices(sp_shell *shell);
 
 /* Workspace sizes in bytes for nfields fields (filter: nfields = total stored components of the

@@ -275,3 +275,21 @@ def test_gradient_is_deterministic():
     a = sh.cartesian_gradient(u).clone()
     for _ in range(3):
         assert torch.equal(sh.cartesian_gradient(u), a)
+
+
+def test_shell_too_large_for_the_plane_kernels_is_refused_and_extreme_small_shells_work():
+    """Maximum size: an antipodal (r, theta) plane pair must fit one SM's shared memory (spshell.h, SIZE LIMIT); the build
+    refuses larger shells with SP_ERR_UNSUPPORTED instead of launching anything.  Minimum size: Nr = Ntheta = 2."""
+    from paper_1104_3408_b200 import Shell
+    from paper_1104_3408_b200.binding import SpError
+    torch = _torch()
+    with pytest.raises(SpError, match="UNSUPPORTED"):
+        Shell(129, 128, 256, 1.5, 9.0, 100)
+    Nr, Nt, Np, L = 2, 2, 4, 1
+    sh = Shell(Nr, Nt, Np, 1.5, 9.0, L)
+    u = np.random.default_rng(2).standard_normal((2, Np, Nt, Nr))
+    got = sh.cartesian_gradient(torch.from_numpy(u).cuda()).cpu().numpy()
+    assert _rel(got, oracle.gradient(u, Nr, Nt, Np, 1.5, 9.0)) < TOL
+    tens = [{"name": "s", "rank": 0, "dims": (), "sym": (-1, -1), "fields": [0]}]
+    gotf = sh.tensor_filter(torch.from_numpy(u).cuda(), tens).cpu().numpy()
+    assert _rel(gotf, oracle.tensor_filter(u, Nr, Nt, Np, L, tens)) < TOL
