@@ -512,7 +512,9 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         PhiGradEpi ge = {du + (size_t)nf * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
         // the fold halves the DMMAs but doubles the rows each warp finishes; measured: it wins from Nphi = 128 upwards
         if (s->gf_ok && Np >= 128) {      // reflection-folded d/dphi with the chain rule in the epilogue
-            const int NC = phi_ncol((int)plane, nf);
+            // 32-column tiles for this kernel at every size (config 4: 0.97 -> 0.88 ms; small states use them anyway)
+            static const int nc_env = [] { const char *e = getenv("SP_PHI_NC"); return e ? atoi(e) : 0; }();
+            const int NC = (nc_env == 64) ? 64 : 32;
             const long ctas = (long)(((int)plane + NC - 1) / NC) * nf;
             // row blocks as in launch_phi_gemm: two CTAs of half the rows when the kernel has an even number of warp rows and many
             // column tiles (config 4: 1.17 -> 0.97 ms)
