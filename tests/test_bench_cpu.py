@@ -25,3 +25,22 @@ def test_flops_per_unit_totals():
         fl = bench.flops_per_unit(synth.config(cid))
         assert fl["grad_dphi"] + fl["grad_rtheta"] == g
         assert fl["filt_analysis"] + fl["filt_theta"] + fl["filt_synthesis"] == f
+
+
+def test_reference_arm_prints_the_contract_line():
+    """`bench.py --impl reference` (the oracle arm) on the smallest config: one JSON line with the contract's keys."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--config", "1", "--steps", "1",
+                          "--warmup", "0"], capture_output=True, text=True, timeout=300, check=True).stdout.strip().splitlines()
+    assert len(out) == 1
+    d = json.loads(out[0])
+    for key in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert key in d, key
+    assert d["impl"] == "reference" and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+    assert d["unit"] == bench.UNIT and d["metric"] == bench.METRIC
