@@ -15,7 +15,11 @@
 #include "kernels_gemm2.cuh"
 
 #define TH_RC 36                        // radii per CTA = 9 column tiles = NT tiles per warp x (9 / NT) warp columns
-#define TH_PKB 37
+// coefficient tile in shared memory, two layouts (measured): NT = 1 (many narrow warps): row pitch 38 (rows t = 0..3 land 6
+// eight-byte slots apart mod 16) and array pitch = 8 mod 16 with the arrays a lane pair (v = 0, 1) reads together as neighbours:
+// conflict-free fragments (config 4: 0.94 -> 0.89 ms); NT = 3: row pitch 37, arrays back to back (config 3: 61 us against 63.5)
+#define TH_PKB_OF(NT) ((NT) == 1 ? 38 : 37)
+#define TH_ARR_OF(NT) (TH_KC * TH_PKB_OF(NT) + ((NT) == 1 ? 8 : 0))
 #define TH_KC 16
 #define TH_STAGES 3
 #define TH_PA 20
@@ -46,7 +50,12 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     const int mg = warp % mgroups, ng = warp / mgroups, nwarps = blockDim.x >> 5;
     const size_t vec = (size_t)Nt * Nr, dofsz = (size_t)MC4 * vec, fsz = (size_t)Nt8 * Nt8;
     const int mca = m, mcb = L + m;                            // rows a_0..a_L, b_1..b_L
-    const int stageA = NMAT * Nt8 * TH_PA, stageB = NARR * TH_KC * TH_PKB;
+    constexpr int TH_PKB = TH_PKB_OF(NT), TH_ARR = TH_ARR_OF(NT);
+    const int stageA = NMAT * Nt8 * TH_PA, stageB = NARR * TH_ARR;
+    // shared-memory slot of source array arr: the pairs a lane pair (v = 0, 1) reads together are neighbours
+    auto slot = [](int arr) { return CPLX ? ((arr == 0) ? 0 : (arr == 2) ? 1 : (arr == 3) ? 2 : 3) : arr; };
+    // offset of (array, row) in a stage of the coefficient tile
+    auto brow = [&](int arr, int r) { return NT == 1 ? slot(arr) * TH_ARR + r * TH_PKB : (arr * TH_KC + r) * TH_PKB; };
     double *As = sm, *Bs = sm + TH_STAGES * stageA;
     const int nrad = min(TH_RC, Nr - k0);
     // source arrays: real: [a_m, b_m]; complex: [a^r, b^r, a^i, b^i]
@@ -71,7 +80,7 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
             const int ii = kc * TH_KC + r;
             const bool rowlive = ii < Nt && !(m == 0 && (arr & 1));                     // b_0 does not exist
             const double *srow = srcR + (size_t)(arr >> 1) * dofsz + (size_t)((arr & 1) ? mcb : mca) * vec + (size_t)ii * Nr;
-            double *drow = bs + row * TH_PKB;
+            double *drow = bs + (NT == 1 ? brow(arr, r) : row * TH_PKB);
             if (rowlive && lane < nrad) cp_async8(drow + lane, srow + lane); else drow[lane] = 0.0;
             if (lane < TH_RC - 32) {
                 if (rowlive && lane + 32 < nrad) cp_async8(drow + 32 + lane, srow + 32 + lane); else drow[32 + lane] = 0.0;
@@ -109,9 +118,9 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
 #pragma unroll
             for (int b = 0; b < NT; b++) {
                 const int kk = (ng * NT + b) * 4 + kq;
-                const double x = bs[(arrX * TH_KC + ks * 4 + t) * TH_PKB + kk];
+                const double x = bs[brow(arrX, ks * 4 + t) + kk];
                 if (CPLX) {
-                    const double y = ysgn * bs[(arrY * TH_KC + ks * 4 + t) * TH_PKB + kk];
+                    const double y = ysgn * bs[brow(arrY, ks * 4 + t) + kk];
                     b1[b] = (m > 0) ? 0.5 * x + y : x;
                     b2[b] = 0.5 * x - y;
                 } else {
@@ -160,6 +169,6 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     }
 }
 
-static inline size_t theta2_smem_bytes(int Nt8, bool cplx) {
-    return (size_t)TH_STAGES * ((size_t)(cplx ? 2 : 1) * Nt8 * TH_PA + (cplx ? 4 : 2) * TH_KC * TH_PKB) * sizeof(double);
+static inline size_t theta2_smem_bytes(int Nt8, bool cplx, int NT = 1) {      // NT = 1 has the larger tile
+    return (size_t)TH_STAGES * ((size_t)(cplx ? 2 : 1) * Nt8 * TH_PA + (cplx ? 4 : 2) * TH_ARR_OF(NT)) * sizeof(double);
 }

@@ -267,7 +267,7 @@ static sp_status launch_theta2(const sp_shell *s, int NT, const std::vector<Thet
     for (int pass = 1; pass >= 0; pass--) {
         const std::vector<ThetaComp2> &lst = pass ? cx : rl;
         st = (fork && pass == 0) ? s->aux : main_st;
-        const size_t sm = theta2_smem_bytes(s->Nt8, pass == 1);
+        const size_t sm = theta2_smem_bytes(s->Nt8, pass == 1, NT);
         for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
             ThetaBatch2 b;
             const int nb = (int)std::min<size_t>(SP_THETA2_BATCH, lst.size() - c0);
