@@ -29,6 +29,12 @@ __device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gmem));
 }
 
+// 8-byte cp.async; with ignore = true the source is not read and zeros are written
+__device__ __forceinline__ void cp_async8_ign(void *smem, const void *gmem, bool ignore) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %2, 0;\n cp.async.ca.shared.global [%0], [%1], 8, p;\n}\n" ::"r"(s), "l"(gmem), "r"((int)ignore));
+}
+
 struct ThetaComp2 { int dof; int n; };
 #define SP_THETA2_BATCH 96
 struct ThetaBatch2 { ThetaComp2 c[SP_THETA2_BATCH]; };
@@ -64,26 +70,45 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     const long dF = CPLX ? -2L * cmp.n * (long)(L + 1) * (long)fsz : 0L;   // F^{-n}_m relative to F^n_m
     const int nchunks = (Nt8 + TH_KC - 1) / TH_KC;
 
+    // loaders.  Their instruction count matters (at 3 K-chunks per CTA they run as often as the tensor loop), so every address
+    // is a pointer or shared-memory offset set up once per chunk and advanced by a constant; dead rows / columns are zero-filled
+    // by cp.async with the ignore-src predicate (no divergent store path).
+    const int hF = tid & 7, rF0 = tid >> 3, rFstep = blockDim.x >> 3;          // F tile: 8 sixteen-byte pieces per row
+    const size_t offAB = (size_t)L * vec;                                       // b_m relative to a_m
+    const double *srcA = srcR + (size_t)mca * vec + lane;                       // a_m rows of the (real part of the) component
+    const bool live0 = lane < nrad, live1 = lane + 32 < nrad, lane_hi = lane < TH_RC - 32;
     auto load_chunk = [&](int kc, int st) {
-        double *as = As + st * stageA;
-        for (int q = tid; q < NMAT * Nt8 * (TH_KC / 2); q += blockDim.x) {
-            const int rr = q >> 3, h = q & 7;                       // TH_KC / 2 = 8 sixteen-byte pieces per row
-            const int mat = (rr >= Nt8) ? 1 : 0, r = rr - mat * Nt8;
-            double *dst = as + rr * TH_PA + 2 * h;
-            if (kc * TH_KC + 2 * h < Nt8) cp_async16(dst, F0 + mat * dF + (size_t)r * Nt8 + kc * TH_KC + 2 * h);
-            else { dst[0] = 0.0; dst[1] = 0.0; }
+        double *as = As + st * stageA + rF0 * TH_PA + 2 * hF;
+        if (kc * TH_KC + 2 * hF < Nt8) {
+            const double *fs = F0 + rF0 * Nt8 + kc * TH_KC + 2 * hF;
+            const int fstep = rFstep * Nt8;
+#pragma unroll 1
+            for (int r = rF0; r < Nt8; r += rFstep, as += rFstep * TH_PA, fs += fstep) {
+                cp_async16(as, fs);
+                if (CPLX) cp_async16(as + Nt8 * TH_PA, fs + dF);
+            }
+        } else {
+#pragma unroll 1
+            for (int r = rF0; r < Nt8; r += rFstep, as += rFstep * TH_PA) {
+                as[0] = 0.0; as[1] = 0.0;
+                if (CPLX) { as[Nt8 * TH_PA] = 0.0; as[Nt8 * TH_PA + 1] = 0.0; }
+            }
         }
         // raw coefficient rows: one (array, latitude) row of 36 radii per warp iteration, lane = radius
-        double *bs = Bs + st * stageB;
-        for (int row = warp; row < NARR * TH_KC; row += nwarps) {
-            const int arr = row / TH_KC, r = row % TH_KC;
-            const int ii = kc * TH_KC + r;
-            const bool rowlive = ii < Nt && !(m == 0 && (arr & 1));                     // b_0 does not exist
-            const double *srow = srcR + (size_t)(arr >> 1) * dofsz + (size_t)((arr & 1) ? mcb : mca) * vec + (size_t)ii * Nr;
-            double *drow = bs + (NT == 1 ? brow(arr, r) : row * TH_PKB);
-            if (rowlive && lane < nrad) cp_async8(drow + lane, srow + lane); else drow[lane] = 0.0;
-            if (lane < TH_RC - 32) {
-                if (rowlive && lane + 32 < nrad) cp_async8(drow + 32 + lane, srow + 32 + lane); else drow[32 + lane] = 0.0;
+        const int kbase = kc * TH_KC;
+        const double *g0 = srcA + (size_t)(kbase + warp) * Nr;
+        double *bs = Bs + st * stageB + lane;
+        const int gstep = nwarps * Nr, sstep = nwarps * TH_PKB;
+#pragma unroll
+        for (int arr = 0; arr < NARR; arr++) {
+            const double *gp = g0 + (arr >> 1) * dofsz + (arr & 1) * offAB;
+            double *sp = bs + brow(arr, warp);
+            const bool arrdead = (m == 0) && (arr & 1);                                 // b_0 does not exist
+#pragma unroll 1
+            for (int r = warp; r < TH_KC; r += nwarps, gp += gstep, sp += sstep) {
+                const bool dead = arrdead || kbase + r >= Nt;
+                cp_async8_ign(sp, gp, dead || !live0);
+                if (lane_hi) cp_async8_ign(sp + 32, gp + 32, dead || !live1);
             }
         }
     };
@@ -104,7 +129,7 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     const int v = g & 1, kq = g >> 1;
     // B-fragment sources of this lane: real: arr v; complex: X = v ? a^i : a^r, Y = v ? b^r : b^i (sign -1 if v)
     const int arrX = CPLX ? (v ? 2 : 0) : v, arrY = CPLX ? (v ? 1 : 3) : 0;
-    const double ysgn = v ? -0.5 : 0.5;
+    const double ysgn = v ? -0.5 : 0.5, xscl = (m > 0) ? 0.5 : 1.0;
     for (int kc = 0; kc < nchunks; kc++) {
         cp_async_wait<TH_STAGES - 2>();
         __syncthreads();
@@ -120,9 +145,9 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
                 const int kk = (ng * NT + b) * 4 + kq;
                 const double x = bs[brow(arrX, ks * 4 + t) + kk];
                 if (CPLX) {
-                    const double y = ysgn * bs[brow(arrY, ks * 4 + t) + kk];
-                    b1[b] = (m > 0) ? 0.5 * x + y : x;
-                    b2[b] = 0.5 * x - y;
+                    const double y = ysgn * bs[brow(arrY, ks * 4 + t) + kk];      // m = 0: the b_0 rows are zero-filled, y = 0
+                    b1[b] = fma(x, xscl, y);
+                    b2[b] = fma(x, xscl, -y);
                 } else {
                     b1[b] = x;
                 }
@@ -140,8 +165,9 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
             }
         }
     }
-    // epilogue: lane owns latitude i = (mg*MT + a)*8 + g and radius k = k0 + (ng*3 + b)*4 + t
-    double *Ro = cout + (size_t)cmp.dof * dofsz, *Io = Ro + dofsz;
+    // epilogue: lane owns latitude i = (mg*MT + a)*8 + g and radius k = k0 + (ng*NT + b)*4 + t; 32-bit offsets from one base
+    double *Ro = cout + (size_t)cmp.dof * dofsz + (size_t)mca * vec + k0;       // a~_m row block of the (real part of the) component
+    const int eAB = (int)offAB, eRI = (int)dofsz;                               // a dof array is far below 2^31 elements
 #pragma unroll
     for (int a = 0; a < MT; a++) {
         const int i = (mg * MT + a) * 8 + g;
@@ -150,20 +176,20 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
         for (int b = 0; b < NT; b++) {
             const int kl = (ng * NT + b) * 4 + t;
             if (kl >= nrad) continue;
-            const size_t off = (size_t)i * Nr + k0 + kl;
+            const int off = i * Nr + kl;
             const double pp = acc[0][a][b][0], qq = acc[0][a][b][1];
             if (!CPLX) {
-                Ro[(size_t)mca * vec + off] = pp;
-                if (m > 0) Ro[(size_t)mcb * vec + off] = qq;
+                Ro[off] = pp;
+                if (m > 0) Ro[off + eAB] = qq;
             } else if (m > 0) {
                 const double ss = acc[NMAT - 1][a][b][0], tt = acc[NMAT - 1][a][b][1];
-                Ro[(size_t)mca * vec + off] = pp + ss;
-                Ro[(size_t)mcb * vec + off] = tt - qq;
-                Io[(size_t)mca * vec + off] = qq + tt;
-                Io[(size_t)mcb * vec + off] = pp - ss;
+                Ro[off] = pp + ss;
+                Ro[off + eAB] = tt - qq;
+                Ro[off + eRI] = qq + tt;
+                Ro[off + eRI + eAB] = pp - ss;
             } else {
                 Ro[off] = pp;
-                Io[off] = qq;
+                Ro[off + eRI] = qq;
             }
         }
     }
