@@ -23,6 +23,11 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
     unsigned s = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
 }
+// 16-byte cp.async; with ignore = true the source is not read and zeros are written
+__device__ __forceinline__ void cp_async16_ign(void *smem, const void *gmem, bool ignore) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %2, 0;\n cp.async.cg.shared.global [%0], [%1], 16, p;\n}\n" ::"r"(s), "l"(gmem), "r"((int)ignore));
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
@@ -63,22 +68,24 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
     const int nchunks = (K + KC - 1) / KC;
     const int colsleft = ncols - c0;                    // > 0, even
 
+    // loaders: per-thread pointers set up once per chunk and advanced by constants (the loader's instruction count is comparable
+    // to the tensor loop's at these short K); rows >= K and columns >= ncols are zero-filled through cp.async's ignore-src
+    const int hA = tid & (KC / 2 - 1), rA0 = tid / (KC / 2), rAstep = blockDim.x / (KC / 2);
+    const int hB = tid % HC, rB0 = tid / HC, rBstep = blockDim.x / HC;
+    const bool coldead = 2 * hB >= colsleft;
+    const long gAstep = (long)rAstep * lda, gBstep = (long)rBstep * sBk;
     auto load_chunk = [&](int kc, int st) {
-        // A chunk: Mpad rows x 8 doubles (4 x 16 B per row); rows and K are zero padded in global memory
-        double *as = As + st * stageA;
-        for (int q = tid; q < Mpad * (KC / 2); q += blockDim.x) {
-            const int r = q / (KC / 2), h = q % (KC / 2);
-            cp_async16(as + r * PA + 2 * h, A + (long)r * lda + kc * KC + 2 * h);
-        }
-        // B chunk: 8 rows x 64 columns (32 x 16 B per row); rows >= K and columns >= ncols are zero-filled
-        double *bs = Bs + st * stageB;
-        for (int q = tid; q < KC * HC; q += blockDim.x) {
-            const int r = q / HC, h = q % HC;
-            const int k = kc * KC + r;
-            double *dst = bs + r * PG_PB + 2 * h;
-            if (k < K && 2 * h < colsleft) cp_async16(dst, Bb + (long)k * sBk + 2 * h);
-            else { dst[0] = 0.0; dst[1] = 0.0; }
-        }
+        // A chunk: Mpad rows x 16 doubles (8 x 16 B per row); rows and K are zero padded in global memory
+        double *as = As + st * stageA + rA0 * PA + 2 * hA;
+        const double *ga = A + (long)rA0 * lda + kc * KC + 2 * hA;
+#pragma unroll 1
+        for (int r = rA0; r < Mpad; r += rAstep, as += rAstep * PA, ga += gAstep) cp_async16(as, ga);
+        // B chunk: 16 rows x NC columns
+        double *bs = Bs + st * stageB + rB0 * PG_PB + 2 * hB;
+        const double *gb = Bb + (long)(kc * KC + rB0) * sBk + 2 * hB;
+#pragma unroll 1
+        for (int r = rB0; r < KC; r += rBstep, bs += rBstep * PG_PB, gb += gBstep)
+            cp_async16_ign(bs, gb, coldead || kc * KC + r >= K);
     };
 
     double acc[MT][2][2];

@@ -43,23 +43,31 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
     const int nchunks = (K + GF_KC - 1) / GF_KC;
     const int mtiles = (M + 7) >> 3;
 
+    // loaders: per-thread pointers set up once per chunk and advanced by constants; dead rows / columns are zero-filled through
+    // cp.async's ignore-src (see k_phi_gemm)
+    const int hA = tid & 3, rA0 = tid >> 2, rAstep = blockDim.x >> 2;          // matrices: 4 x 16 B per row
+    const int hB = tid % HC, rB0 = tid / HC, rBstep = blockDim.x / HC;         // field rows: NC/2 x 16 B per row
+    const bool coldead = 2 * hB >= colsleft;
+    const long gAstep = (long)rAstep * lda, gBstep = (long)rBstep * sUj;
     auto load_chunk = [&](int kc, int st) {
-        double *as = As + st * stageA;
-        for (int q = tid; q < 2 * Mpad * 4; q += blockDim.x) {          // both matrices, 4 x 16 B per row
-            const int rr = q >> 2, hh = q & 3;
-            const int mat = rr >= Mpad, r = rr - mat * Mpad;
-            cp_async16(as + rr * GF_PA + 2 * hh, (mat ? Gp : Gm) + (long)r * lda + kc * GF_KC + 2 * hh);
+        double *as = As + st * stageA + rA0 * GF_PA + 2 * hA;
+        const long ao = (long)rA0 * lda + kc * GF_KC + 2 * hA;
+        const double *gm = Gm + ao, *gp = Gp + ao;
+#pragma unroll 1
+        for (int r = rA0; r < Mpad; r += rAstep, as += rAstep * GF_PA, gm += gAstep, gp += gAstep) {
+            cp_async16(as, gm);
+            cp_async16(as + Mpad * GF_PA, gp);
         }
-        double *bs = Bs + st * stageB;
-        for (int q = tid; q < 2 * GF_KC * HC; q += blockDim.x) {   // rows jj and J - jj, NC/2 x 16 B per row
-            const int rr = q / HC, hh = q % HC;
-            const int mir = rr >= GF_KC, r = rr - mir * GF_KC;
+        // rows jj (ascending) and their mirrors J - jj (descending; J -> 0)
+        double *bs = Bs + st * stageB + rB0 * GF_PB + 2 * hB;
+        const int jj0 = kc * GF_KC + rB0;
+        const double *gu = Ub + (long)jj0 * sUj + 2 * hB, *gv = Ub + (long)(J - jj0) * sUj + 2 * hB;
+#pragma unroll 1
+        for (int r = rB0; r < GF_KC; r += rBstep, bs += rBstep * GF_PB, gu += gBstep, gv -= gBstep) {
             const int jj = kc * GF_KC + r;
-            int j = mir ? J - jj : jj;
-            if (j == J) j = 0;
-            double *dst = bs + rr * GF_PB + 2 * hh;
-            if (jj < K && 2 * hh < colsleft) cp_async16(dst, Ub + (long)j * sUj + 2 * hh);
-            else { dst[0] = 0.0; dst[1] = 0.0; }
+            const bool dead = coldead || jj >= K;
+            cp_async16_ign(bs, gu, dead);
+            cp_async16_ign(bs + GF_KC * GF_PB, jj == 0 ? gu : gv, dead);
         }
     };
 
