@@ -88,6 +88,14 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
             cp_async16_ign(bs, gb, coldead || kc * KC + r >= K);
     };
 
+    // EPI_GRAD: 1/(r sin th) of the column pair this thread walks in phase 2 of the epilogue (q % HC = tid % HC because HC divides
+    // the block size), loaded now so that the epilogue does not start with a global-load round trip
+    double2 fcol = make_double2(0.0, 0.0);
+    if (EPI_GRAD) {
+        const int c = c0 + 2 * (tid % HC);                          // flat (k, i) column: c = k + Nr i
+        if (c < ncols) { const int i = c / ge.Nr, k = c - i * ge.Nr; fcol.x = __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i); }
+        if (c + 1 < ncols) { const int i = (c + 1) / ge.Nr, k = c + 1 - i * ge.Nr; fcol.y = __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i); }
+    }
     double acc[MT][2][2];
 #pragma unroll
     for (int a = 0; a < MT; a++)
@@ -133,32 +141,20 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
             }
         }
     } else {
-        // two phases.  (1) every lane scales its accumulators to c = d_phi u /(r sin th) and parks them in shared memory (the
-        // pipeline buffers are free now) as an [M][NC] tile.  (2) all threads walk the tile row-contiguously: coalesced 16-byte
-        // loads of W, coalesced stores of d_x and d_y, several independent loads in flight per thread.
+        // two phases.  (1) every lane parks its accumulators (d_phi u) in shared memory (the pipeline buffers are free now) as an
+        // [M][NC] tile.  (2) all threads walk the tile row-contiguously: c = d_phi u /(r sin th) with the thread's column factors,
+        // coalesced 16-byte loads of W, coalesced stores of d_x and d_y, several independent loads in flight per thread.
         cp_async_wait<0>();
         __syncthreads();
         double *cs = sm;
         double *Yb = ge.Y + (long)blockIdx.y * ge.sYb + c0;
-        {
-            double f[2][2];                    // 1/(r sin th) of the lane's four columns
+#pragma unroll
+        for (int a = 0; a < MT; a++) {
+            const int row = (mg * MT + a) * 8 + g;                       // longitude j
+            if (row >= M) continue;
 #pragma unroll
             for (int b = 0; b < 2; b++)
-#pragma unroll
-                for (int e = 0; e < 2; e++) {
-                    const int c = c0 + ng * 16 + b * 8 + 2 * t + e;        // flat (k, i) column: c = k + Nr i
-                    const int i = c / ge.Nr, k = c - i * ge.Nr;
-                    f[b][e] = (c < ncols) ? __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i) : 0.0;
-                }
-#pragma unroll
-            for (int a = 0; a < MT; a++) {
-                const int row = (mg * MT + a) * 8 + g;                       // longitude j
-                if (row >= M) continue;
-#pragma unroll
-                for (int b = 0; b < 2; b++)
-                    *reinterpret_cast<double2 *>(cs + row * PG_PC + ng * 16 + b * 8 + 2 * t) =
-                        make_double2(acc[a][b][0] * f[b][0], acc[a][b][1] * f[b][1]);
-            }
+                *reinterpret_cast<double2 *>(cs + row * PG_PC + ng * 16 + b * 8 + 2 * t) = make_double2(acc[a][b][0], acc[a][b][1]);
         }
         __syncthreads();
         const int npair = min(NC, colsleft) >> 1;
@@ -177,7 +173,8 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
 #pragma unroll
             for (int z = 0; z < UNR; z++) {
                 if (!ok[z]) continue;
-                const double2 c = *reinterpret_cast<const double2 *>(cs + row[z] * PG_PC + 2 * cp2[z]);
+                double2 c = *reinterpret_cast<const double2 *>(cs + row[z] * PG_PC + 2 * cp2[z]);
+                c.x *= fcol.x; c.y *= fcol.y;
                 const double sp = __ldg(ge.sin_p + row[z]), cp = __ldg(ge.cos_p + row[z]);
                 *reinterpret_cast<double2 *>(Cb + (long)row[z] * sCm + 2 * cp2[z]) = make_double2(cp * w[z].x - sp * c.x, cp * w[z].y - sp * c.y);
                 *reinterpret_cast<double2 *>(Yb + (long)row[z] * sCm + 2 * cp2[z]) = make_double2(sp * w[z].x + cp * c.x, sp * w[z].y + cp * c.y);

@@ -71,6 +71,14 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
         }
     };
 
+    // 1/(r sin th) of the column pair this thread walks in phase 2 of the epilogue (q % HC = tid % HC because HC divides the
+    // block size), loaded now so that the epilogue does not start with a global-load round trip
+    double2 fcol = make_double2(0.0, 0.0);
+    {
+        const int c = c0 + 2 * (tid % HC);                              // flat (k, i) column: c = k + Nr i
+        if (c < ncols) { const int i = c / ge.Nr, k = c - i * ge.Nr; fcol.x = __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i); }
+        if (c + 1 < ncols) { const int i = (c + 1) / ge.Nr, k = c + 1 - i * ge.Nr; fcol.y = __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i); }
+    }
     double aO[MT][2][2], aE[MT][2][2];
 #pragma unroll
     for (int a = 0; a < MT; a++)
@@ -110,36 +118,24 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
             }
         }
     }
-    // ---- epilogue, two phases.  (1) every lane scales its accumulators to c = d_phi u /(r sin th) and parks them in shared
-    // memory (the pipeline buffers are free now) as a [J][64] tile.  (2) all threads walk the tile row-contiguously: coalesced
-    // 16-byte loads of W, coalesced stores of d_x and d_y, many independent loads in flight per thread.
+    // ---- epilogue, two phases.  (1) every lane unfolds its accumulators to d_phi u and parks them in shared memory (the pipeline
+    // buffers are free now) as a [J][64] tile.  (2) all threads walk the tile row-contiguously: c = d_phi u /(r sin th) with the
+    // thread's column factors, coalesced 16-byte loads of W, coalesced stores of d_x and d_y, many independent loads in flight.
     cp_async_wait<0>();
     __syncthreads();
     double *cs = sm;                                                        // [2 Mpad][GF_PC]: rows j', then their mirrors J - j'
-    {
-        double f[2][2];
 #pragma unroll
-        for (int b = 0; b < 2; b++)
+    for (int a = 0; a < MT; a++) {
+        const int row = (mg * MT + a) * 8 + g;                          // local row; j' = r0 + row in [0, h]
+        if (row >= M) continue;
+        const bool mirrored = r0 + row > 0 && r0 + row < h;
 #pragma unroll
-            for (int e = 0; e < 2; e++) {
-                const int c = c0 + ng * 16 + b * 8 + 2 * t + e;            // flat (k, i) column: c = k + Nr i
-                const int i = c / ge.Nr, k = c - i * ge.Nr;
-                f[b][e] = (c < ncols) ? __ldg(ge.inv_r + k) * __ldg(ge.inv_sin_t + i) : 0.0;
-            }
-#pragma unroll
-        for (int a = 0; a < MT; a++) {
-            const int row = (mg * MT + a) * 8 + g;                          // local row; j' = r0 + row in [0, h]
-            if (row >= M) continue;
-            const bool mirrored = r0 + row > 0 && r0 + row < h;
-#pragma unroll
-            for (int b = 0; b < 2; b++) {
-                const int col = ng * 16 + b * 8 + 2 * t;
-                *reinterpret_cast<double2 *>(cs + row * GF_PC + col) =
-                    make_double2((aO[a][b][0] + aE[a][b][0]) * f[b][0], (aO[a][b][1] + aE[a][b][1]) * f[b][1]);
-                if (mirrored)
-                    *reinterpret_cast<double2 *>(cs + (Mpad + row) * GF_PC + col) =
-                        make_double2((aO[a][b][0] - aE[a][b][0]) * f[b][0], (aO[a][b][1] - aE[a][b][1]) * f[b][1]);
-            }
+        for (int b = 0; b < 2; b++) {
+            const int col = ng * 16 + b * 8 + 2 * t;
+            *reinterpret_cast<double2 *>(cs + row * GF_PC + col) = make_double2(aO[a][b][0] + aE[a][b][0], aO[a][b][1] + aE[a][b][1]);
+            if (mirrored)
+                *reinterpret_cast<double2 *>(cs + (Mpad + row) * GF_PC + col) =
+                    make_double2(aO[a][b][0] - aE[a][b][0], aO[a][b][1] - aE[a][b][1]);
         }
     }
     __syncthreads();
@@ -163,7 +159,8 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
 #pragma unroll
         for (int z = 0; z < UNR; z++) {
             if (!ok[z]) continue;
-            const double2 c = *reinterpret_cast<const double2 *>(cs + lrow[z] * GF_PC + 2 * cp2[z]);
+            double2 c = *reinterpret_cast<const double2 *>(cs + lrow[z] * GF_PC + 2 * cp2[z]);
+            c.x *= fcol.x; c.y *= fcol.y;
             const double sp = __ldg(ge.sin_p + row[z]), cp = __ldg(ge.cos_p + row[z]);
             *reinterpret_cast<double2 *>(Xb + (long)row[z] * sUj + 2 * cp2[z]) = make_double2(cp * w[z].x - sp * c.x, cp * w[z].y - sp * c.y);
             *reinterpret_cast<double2 *>(Yb + (long)row[z] * sUj + 2 * cp2[z]) = make_double2(sp * w[z].x + cp * c.x, sp * w[z].y + cp * c.y);
