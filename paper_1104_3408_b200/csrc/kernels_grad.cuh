@@ -340,16 +340,24 @@ __global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_r
     const size_t npts = (size_t)Nr * Nt * Np, plane = (size_t)Nr * Nt;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
 
-    // planes of one item: one latitude row per warp iteration, 8-byte cp.async into the padded pitch
+    // planes of one item: a plane is Nr*Nt contiguous doubles in global memory; thread e, e + blockDim, .. copies element e
+    // (8-byte cp.async, coalesced) to row i = e / Nr, column k = e % Nr of the padded pitch.  (i, k) advance incrementally: the
+    // loader's instruction count matters as much as the tensor loop's (it was 19 % of the kernel's instructions as a nested
+    // row / column loop)
+    const int ldi = blockDim.x / Nr, ldk = blockDim.x - ldi * Nr, lstep = ldi * PU + ldk;
+    const int li0 = threadIdx.x / Nr, lk0 = threadIdx.x - li0 * Nr, nplane = Nr * Nt;
     auto issue_planes = [&](int it, double *B0) {
         const int mu_ = it / Nt, j_ = it - mu_ * Nt;
-        const double *u0 = p.u + mu_ * npts + (size_t)j_ * plane, *u1 = u0 + (size_t)Nt * plane;
-        double *B1 = B0 + planesz;
-        for (int i = warp; i < Nt; i += nwarps)
-            for (int k = lane; k < Nr; k += 32) {
-                cp_async8g(B0 + i * PU + k, u0 + (size_t)i * Nr + k);
-                cp_async8g(B1 + i * PU + k, u1 + (size_t)i * Nr + k);
-            }
+        const double *u0 = p.u + mu_ * npts + (size_t)j_ * plane + threadIdx.x, *u1 = u0 + (size_t)Nt * plane;
+        double *s0 = B0 + li0 * PU + lk0, *s1 = s0 + planesz;
+        int k = lk0;
+#pragma unroll 1
+        for (int e = threadIdx.x; e < nplane; e += blockDim.x) {
+            cp_async8g(s0, u0);
+            cp_async8g(s1, u1);
+            u0 += blockDim.x; u1 += blockDim.x; k += ldk; s0 += lstep; s1 += lstep;
+            if (k >= Nr) { k -= Nr; s0 += PU - Nr; s1 += PU - Nr; }
+        }
     };
     // padding (columns >= Nr, rows >= Nt) of every buffer: zero, once
     for (int bq = 0; bq < 2 * NBUF; bq++) {
