@@ -239,6 +239,12 @@ static bool sp_join(const sp_shell *s, cudaStream_t st) {
     return cudaEventRecord(s->ev_join, s->aux) == cudaSuccess && cudaStreamWaitEvent(st, s->ev_join, 0) == cudaSuccess;
 }
 
+// smallest Nphi at which d/dphi runs reflection-folded (k_phi_grad_fold); SP_DPHI_FOLD_MIN overrides (experiments)
+static int sp_dphi_fold_min() {
+    static const int v = [] { const char *e = getenv("SP_DPHI_FOLD_MIN"); return e ? atoi(e) : 128; }();
+    return v;
+}
+
 // theta step launcher: NT = 3 or 1 column tiles per warp (see kernels_theta2.cuh)
 static void theta2_tiling(const sp_shell *s, int NT, int &MT, int &mgroups) {
     const int mtiles = s->Nt8 / 8, ngc = 9 / NT;
@@ -438,7 +444,7 @@ extern "C" sp_status sp_get_tuning(const sp_shell *s, int out[4]) {
     if (!s->built) return SP_ERR_NOT_BUILT;
     out[0] = s->theta_NT;
     out[1] = s->gradKT;
-    out[2] = (s->gf_ok && s->Np >= 128) ? 1 : 0;
+    out[2] = (s->gf_ok && s->Np >= sp_dphi_fold_min()) ? 1 : 0;
     out[3] = (s->grad3_ctas[1] > 0) ? 2 : 1;
     return SP_OK;
 }
@@ -511,7 +517,7 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         sp_mark(s, st, 1);
         PhiGradEpi ge = {du + (size_t)nf * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
         // the fold halves the DMMAs but doubles the rows each warp finishes; measured: it wins from Nphi = 128 upwards
-        if (s->gf_ok && Np >= 128) {      // reflection-folded d/dphi with the chain rule in the epilogue
+        if (s->gf_ok && Np >= sp_dphi_fold_min()) {      // reflection-folded d/dphi with the chain rule in the epilogue
             // 32-column tiles for this kernel at every size (config 4: 0.97 -> 0.88 ms; small states use them anyway)
             static const int nc_env = [] { const char *e = getenv("SP_PHI_NC"); return e ? atoi(e) : 0; }();
             const int NC = (nc_env == 64) ? 64 : 32;
