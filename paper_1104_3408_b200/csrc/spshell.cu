@@ -343,6 +343,7 @@ sp_status sp_configure_kernels(sp_shell *s) {
         {
             const int nt3 = itiles * ((ktiles + KT - 1) / KT);
             s->grad3_nwarps = (KT == 3) ? std::min(nt3, 12) : std::min(nt3, 6);
+            if (const char *e = getenv("SP_GRAD_NWARPS")) { const int w = atoi(e); if (w >= 1 && w <= (KT == 3 ? 12 : 6)) s->grad3_nwarps = std::min(nt3, w); }   // tuning override
             const int thr = s->grad3_nwarps * 32;
             for (int nb = 1; nb <= 2; nb++) {
                 s->grad3_ctas[nb - 1] = 0;
@@ -363,6 +364,7 @@ sp_status sp_configure_kernels(sp_shell *s) {
 #undef SP_G3
 #undef SP_G3P
                 s->grad3_ctas[nb - 1] = occ;
+                if (const char *e = getenv("SP_GRAD_CTAS")) { const int c = atoi(e); if (c >= 1 && c < occ) s->grad3_ctas[nb - 1] = c; }   // tuning override: resident CTAs per SM
             }
         }
     }
