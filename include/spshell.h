@@ -160,8 +160,9 @@ sp_status sp_probe_fp64_peak(int mode, double *tflops_out);
 sp_status sp_profile_enable(sp_shell *shell, int on);
 sp_status sp_profile_read(const sp_shell *shell, double *ms7_host);
 
-/* Kernel variants sp_build_matrices selected for this shell (reporting only): out[0] = column tiles per warp of the theta
- * kernel (3 or 1, chosen by a timing run at build; 0 = generic kernel), out[1] = radial tiles per warp task of the
+/* Kernel variants sp_build_matrices selected for this shell (reporting only): out[0] = variant of the theta kernel chosen
+ * by a timing run at build: NT + 20 * (rsplit - 1) with NT = 3 or 1 column tiles per warp and rsplit = 1 or 2 row blocks of
+ * latitudes per (component, m, radial block), i.e. 3, 1, 23 or 21 (0 = generic kernel), out[1] = radial tiles per warp task of the
  * (r,theta) gradient kernel (3 or 5), out[2] = 1 if d/dphi uses the reflection-folded kernel, out[3] = 2 if the
  * double-buffered variant of the persistent (r,theta) kernel fits (it is used by calls with at least three waves of planes).  SP_ERR_NOT_BUILT before sp_build_matrices. */
 sp_status sp_get_tuning(const sp_shell *shell, int out[4]);

@@ -44,20 +44,23 @@ struct ThetaBatch2 { ThetaComp2 c[SP_THETA2_BATCH]; };
 // three times as many warps with a third of the registers).  Which one is faster depends on the grid; sp_build_matrices
 // times both on the device and keeps the winner.
 template <int MT, int NT, bool CPLX>
-__global__ void __launch_bounds__(NT == 3 ? 512 : 896, 1)
-k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt8, int Nr, int MC4, int mgroups,
+__global__ void __launch_bounds__(NT == 3 ? 384 : 896, 1)
+k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt8, int Nr, int MC4, int mgroups, int rsplit,
          const double *__restrict__ coef, double *__restrict__ cout) {
     extern __shared__ __align__(16) double sm[];
     constexpr int NMAT = CPLX ? 2 : 1, NARR = CPLX ? 4 : 2;
     const ThetaComp2 cmp = comps.c[blockIdx.y];
     const int m = blockIdx.x;
-    const int k0 = blockIdx.z * TH_RC;
+    // blockIdx.z = radial block * rsplit + row block: with rsplit = 2 a CTA owns half of the latitudes (rows of F^n_m), so its F tile
+    // halves and two CTAs share an SM at large Ntheta; both row blocks read the same coefficient rows
+    const int zr = blockIdx.z % rsplit, k0 = (blockIdx.z / rsplit) * TH_RC;
+    const int Nt8c = Nt8 / rsplit, r0 = zr * Nt8c;                  // rows of this CTA
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp % mgroups, ng = warp / mgroups, nwarps = blockDim.x >> 5;
     const size_t vec = (size_t)Nt * Nr, dofsz = (size_t)MC4 * vec, fsz = (size_t)Nt8 * Nt8;
     const int mca = m, mcb = L + m;                            // rows a_0..a_L, b_1..b_L
     constexpr int TH_PKB = TH_PKB_OF(NT), TH_ARR = TH_ARR_OF(NT);
-    const int stageA = NMAT * Nt8 * TH_PA, stageB = NARR * TH_ARR;
+    const int stageA = NMAT * Nt8c * TH_PA, stageB = NARR * TH_ARR;
     // shared-memory slot of source array arr: the pairs a lane pair (v = 0, 1) reads together are neighbours
     auto slot = [](int arr) { return CPLX ? ((arr == 0) ? 0 : (arr == 2) ? 1 : (arr == 3) ? 2 : 3) : arr; };
     // offset of (array, row) in a stage of the coefficient tile
@@ -80,18 +83,18 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     auto load_chunk = [&](int kc, int st) {
         double *as = As + st * stageA + rF0 * TH_PA + 2 * hF;
         if (kc * TH_KC + 2 * hF < Nt8) {
-            const double *fs = F0 + rF0 * Nt8 + kc * TH_KC + 2 * hF;
+            const double *fs = F0 + (r0 + rF0) * Nt8 + kc * TH_KC + 2 * hF;
             const int fstep = rFstep * Nt8;
 #pragma unroll 1
-            for (int r = rF0; r < Nt8; r += rFstep, as += rFstep * TH_PA, fs += fstep) {
+            for (int r = rF0; r < Nt8c; r += rFstep, as += rFstep * TH_PA, fs += fstep) {
                 cp_async16(as, fs);
-                if (CPLX) cp_async16(as + Nt8 * TH_PA, fs + dF);
+                if (CPLX) cp_async16(as + Nt8c * TH_PA, fs + dF);
             }
         } else {
 #pragma unroll 1
-            for (int r = rF0; r < Nt8; r += rFstep, as += rFstep * TH_PA) {
+            for (int r = rF0; r < Nt8c; r += rFstep, as += rFstep * TH_PA) {
                 as[0] = 0.0; as[1] = 0.0;
-                if (CPLX) { as[Nt8 * TH_PA] = 0.0; as[Nt8 * TH_PA + 1] = 0.0; }
+                if (CPLX) { as[Nt8c * TH_PA] = 0.0; as[Nt8c * TH_PA + 1] = 0.0; }
             }
         }
         // raw coefficient rows: one (array, latitude) row of 36 radii per warp iteration, lane = radius
@@ -158,19 +161,19 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
 #pragma unroll
                 for (int b = 0; b < NT; b++) dmma(acc[0][a][b][0], acc[0][a][b][1], a1, b1[b]);
                 if (CPLX) {
-                    const double a2 = as[(Nt8 + a * 8) * TH_PA + ks * 4];
+                    const double a2 = as[(Nt8c + a * 8) * TH_PA + ks * 4];
 #pragma unroll
                     for (int b = 0; b < NT; b++) dmma(acc[NMAT - 1][a][b][0], acc[NMAT - 1][a][b][1], a2, b2[b]);
                 }
             }
         }
     }
-    // epilogue: lane owns latitude i = (mg*MT + a)*8 + g and radius k = k0 + (ng*NT + b)*4 + t; 32-bit offsets from one base
+    // epilogue: lane owns latitude i = r0 + (mg*MT + a)*8 + g and radius k = k0 + (ng*NT + b)*4 + t; 32-bit offsets from one base
     double *Ro = cout + (size_t)cmp.dof * dofsz + (size_t)mca * vec + k0;       // a~_m row block of the (real part of the) component
     const int eAB = (int)offAB, eRI = (int)dofsz;                               // a dof array is far below 2^31 elements
 #pragma unroll
     for (int a = 0; a < MT; a++) {
-        const int i = (mg * MT + a) * 8 + g;
+        const int i = r0 + (mg * MT + a) * 8 + g;
         if (i >= Nt) continue;
 #pragma unroll
         for (int b = 0; b < NT; b++) {
@@ -195,6 +198,6 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     }
 }
 
-static inline size_t theta2_smem_bytes(int Nt8, bool cplx, int NT = 1) {      // NT = 1 has the larger tile
+static inline size_t theta2_smem_bytes(int Nt8, bool cplx, int NT = 1) {      // NT = 1 has the larger tile; Nt8 = rows per CTA
     return (size_t)TH_STAGES * ((size_t)(cplx ? 2 : 1) * Nt8 * TH_PA + (cplx ? 4 : 2) * TH_ARR_OF(NT)) * sizeof(double);
 }

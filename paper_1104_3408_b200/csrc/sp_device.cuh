@@ -35,7 +35,7 @@ struct sp_shell {
     double *d_gm = nullptr, *d_gp = nullptr;
     int gf_Mpad = 0, gf_lda = 0, gf_mg = 0;
     bool gf_ok = false;
-    int theta_NT = 0;             // column tiles per warp of k_theta2 chosen at build time (3 or 1; 0: generic kernel)
+    int theta_NT = 0;             // k_theta2 variant chosen at build time: NT + 20 * (rsplit - 1), NT = 3 or 1 column tiles per warp, rsplit = 1 or 2 row blocks (3, 1, 23, 21; 0: generic kernel)
     PhiMat m_ac, m_as, m_sc, m_ss;   // analysis cos [L+1][J/2+1], sin [L][J/2-1]; synthesis cos [J/2+1][L+1], sin [J/2-1][L]
     double *d_inv_r = nullptr, *d_sin_t = nullptr, *d_cos_t = nullptr, *d_inv_sin_t = nullptr, *d_sin_p = nullptr,
            *d_cos_p = nullptr;     // Jacobian / triad factors                          (eq. 6, 51)

@@ -245,22 +245,28 @@ static int sp_dphi_fold_min() {
     return v;
 }
 
-// theta step launcher: NT = 3 or 1 column tiles per warp (see kernels_theta2.cuh)
-static void theta2_tiling(const sp_shell *s, int NT, int &MT, int &mgroups) {
-    const int mtiles = s->Nt8 / 8, ngc = 9 / NT;
+// theta step launcher.  Variant code v = NT + 20 * (rsplit - 1): NT = 3 or 1 column tiles per warp, rsplit = 1 or 2 row blocks
+// per (component, m, radial block) (see kernels_theta2.cuh): 3, 1, 23, 21
+static inline int th_NT(int v) { return v % 20; }
+static inline int th_rsplit(int v) { return v / 20 + 1; }
+static void theta2_tiling(const sp_shell *s, int v, int &MT, int &mgroups) {
+    const int NT = th_NT(v), mtiles = s->Nt8 / 8 / th_rsplit(v), ngc = 9 / NT;
     MT = (mtiles % 3 == 0) ? 3 : (mtiles % 4 == 0) ? 4 : (mtiles < 3 ? mtiles : 3);
-    if (((mtiles + MT - 1) / MT) * ngc > (NT == 3 ? 16 : 28) && mtiles % 4 == 0) MT = 4;
+    if (((mtiles + MT - 1) / MT) * ngc > (NT == 3 ? 12 : 28) && mtiles % 4 == 0) MT = 4;
     mgroups = (mtiles + MT - 1) / MT;
 }
-static bool theta2_fits(const sp_shell *s, int NT) {
+static bool theta2_fits(const sp_shell *s, int v) {
+    const int NT = th_NT(v), rs = th_rsplit(v);
+    if ((s->Nt8 / 8) % rs != 0 || s->Nt8 / rs < 8) return false;
     int MT, mg;
-    theta2_tiling(s, NT, MT, mg);
-    return mg * (9 / NT) <= (NT == 3 ? 16 : 28) && theta2_smem_bytes(s->Nt8, true) <= 227 * 1024;
+    theta2_tiling(s, v, MT, mg);
+    return mg * (9 / NT) <= (NT == 3 ? 12 : 28) && theta2_smem_bytes(s->Nt8 / rs, true, NT) <= 227 * 1024;      // launch bounds of k_theta2
 }
-static sp_status launch_theta2(const sp_shell *s, int NT, const std::vector<ThetaComp2> &rl, const std::vector<ThetaComp2> &cx,
+static sp_status launch_theta2(const sp_shell *s, int v, const std::vector<ThetaComp2> &rl, const std::vector<ThetaComp2> &cx,
                                const double *coef1, double *coef2, cudaStream_t st) {
+    const int NT = th_NT(v), rsplit = th_rsplit(v);
     int MT, mgroups;
-    theta2_tiling(s, NT, MT, mgroups);
+    theta2_tiling(s, v, MT, mgroups);
     const dim3 block(mgroups * (9 / NT) * 32);
     const int gz = (s->Nr + TH_RC - 1) / TH_RC;
     // the real and the complex components are independent: the (shorter) real launch runs on the side stream, so CTAs of
@@ -273,15 +279,15 @@ static sp_status launch_theta2(const sp_shell *s, int NT, const std::vector<Thet
     for (int pass = 1; pass >= 0; pass--) {
         const std::vector<ThetaComp2> &lst = pass ? cx : rl;
         st = (fork && pass == 0) ? s->aux : main_st;
-        const size_t sm = theta2_smem_bytes(s->Nt8, pass == 1, NT);
+        const size_t sm = theta2_smem_bytes(s->Nt8 / rsplit, pass == 1, NT);
         for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
             ThetaBatch2 b;
             const int nb = (int)std::min<size_t>(SP_THETA2_BATCH, lst.size() - c0);
             for (int q = 0; q < nb; q++) b.c[q] = lst[c0 + q];
-            const dim3 grid(s->L + 1, nb, gz);
+            const dim3 grid(s->L + 1, nb, gz * rsplit);
 #define SP_TH2(MTV, NTV)                                                                                                        \
-    if (pass) k_theta2<MTV, NTV, true><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, coef1, coef2); \
-    else k_theta2<MTV, NTV, false><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, coef1, coef2);
+    if (pass) k_theta2<MTV, NTV, true><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, rsplit, coef1, coef2); \
+    else k_theta2<MTV, NTV, false><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, rsplit, coef1, coef2);
 #define SP_TH2M(NTV)                                                                                     \
     switch (MT) { case 1: SP_TH2(1, NTV) break; case 2: SP_TH2(2, NTV) break; case 3: SP_TH2(3, NTV) break; default: SP_TH2(4, NTV) break; }
             if (NT == 3) { SP_TH2M(3) } else { SP_TH2M(1) }
@@ -404,38 +410,45 @@ sp_status sp_configure_kernels(sp_shell *s) {
     SP_CUDA(cudaFuncSetAttribute(k_theta2<MTV, NTV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
         SP_TA(1, 3) SP_TA(2, 3) SP_TA(3, 3) SP_TA(4, 3) SP_TA(1, 1) SP_TA(2, 1) SP_TA(3, 1) SP_TA(4, 1)
 #undef SP_TA
-        // measure, don't guess: time both warp tilings on scratch data shaped like a GHG state (12 real + 18 complex
-        // components = 48 coefficient arrays) and keep the winner
-        const bool ok3 = theta2_fits(s, 3), ok1 = theta2_fits(s, 1);
+        // measure, don't guess: time the candidate variants (warp tilings NT = 3 / 1, without and with the row-block split: codes 3, 1,
+        // 23, 21) on scratch data shaped like a GHG state (12 real + 18 complex components = 48 coefficient arrays), keep the winner
+        const int cand[4] = {3, 1, 23, 21};
+        bool ok[4];
+        int nok = 0, only = 0;
         const char *env = getenv("SP_THETA_NT");          // tuning override (profiling: a run under ncu distorts the timing below)
         const int forced = env ? atoi(env) : 0;
-        if (forced == 3 && ok3) s->theta_NT = 3;
-        else if (forced == 1 && ok1) s->theta_NT = 1;
-        else if (ok3 && !ok1) s->theta_NT = 3;
-        else if (ok1 && !ok3) s->theta_NT = 1;
-        else if (ok1 && ok3) {
+        for (int v = 0; v < 4; v++) {
+            ok[v] = theta2_fits(s, cand[v]);
+            if (ok[v]) { nok++; only = cand[v]; }
+            if (ok[v] && forced == cand[v]) s->theta_NT = forced;
+        }
+        if (s->theta_NT == 0 && nok == 1) s->theta_NT = only;
+        if (s->theta_NT == 0 && nok > 1) {
             const size_t dofsz = (size_t)s->MC4 * s->Nt * s->Nr;
             double *scr = nullptr;
             const int nscr = 48;
-            if (cudaMalloc((void **)&scr, 2 * nscr * dofsz * sizeof(double)) != cudaSuccess) { cudaGetLastError(); s->theta_NT = 3; return SP_OK; }
+            if (cudaMalloc((void **)&scr, 2 * nscr * dofsz * sizeof(double)) != cudaSuccess) { cudaGetLastError(); s->theta_NT = ok[0] ? 3 : only; return SP_OK; }
             SP_CUDA(cudaMemset(scr, 0, 2 * nscr * dofsz * sizeof(double)));
             std::vector<ThetaComp2> rl, cx;
             for (int q = 0; q < 12; q++) rl.push_back({q, 0});
             for (int q = 0; q < 18; q++) cx.push_back({12 + 2 * q, 1 + q % 3});
             cudaEvent_t e0, e1;
             SP_CUDA(cudaEventCreate(&e0)); SP_CUDA(cudaEventCreate(&e1));
-            float best[2] = {1e30f, 1e30f};
+            float best[4] = {1e30f, 1e30f, 1e30f, 1e30f};
             for (int rep = 0; rep < 4; rep++)
-                for (int v = 0; v < 2; v++) {
+                for (int v = 0; v < 4; v++) {
+                    if (!ok[v]) continue;
                     cudaEventRecord(e0);
-                    launch_theta2(s, v ? 1 : 3, rl, cx, scr, scr + nscr * dofsz, 0);
+                    launch_theta2(s, cand[v], rl, cx, scr, scr + nscr * dofsz, 0);
                     cudaEventRecord(e1);
                     if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(scr); return SP_ERR_CUDA; }
                     float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
                     if (rep > 0 && ms < best[v]) best[v] = ms;
                 }
             cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(scr);
-            s->theta_NT = best[1] < best[0] ? 1 : 3;
+            int bv = -1;
+            for (int v = 0; v < 4; v++) if (ok[v] && (bv < 0 || best[v] < best[bv])) bv = v;
+            s->theta_NT = cand[bv];
         }
     }
     return SP_OK;

@@ -298,6 +298,8 @@ def test_shell_too_large_for_the_plane_kernels_is_refused_and_extreme_small_shel
 @pytest.mark.parametrize("env", [
     {"SP_THETA_NT": "1", "SP_GRAD_NWARPS": "2", "SP_GRAD_CTAS": "1", "SP_DPHI_FOLD_MIN": "16", "SP_PHI_NC": "32"},
     {"SP_THETA_NT": "3", "SP_GRAD_KT": "3", "SP_GRAD_NWARPS": "4", "SP_PHI_NC": "64", "SP_PHI_MSPLIT": "1"},
+    {"SP_THETA_NT": "23"},
+    {"SP_THETA_NT": "21", "SP_PHI_MSPLIT": "2"},
 ])
 def test_tuning_overrides_keep_parity(env):
     """Every kernel variant the environment overrides can select (README, "tuning overrides") computes the same numbers: the
@@ -306,7 +308,8 @@ def test_tuning_overrides_keep_parity(env):
     import subprocess
     import sys
     child = dict(os.environ, **env)
-    sel = "test_gradient_full or test_filter_full or test_every_tensor_type_ragged_grids or test_gradient_sampled_full_size"
+    sel = ("test_gradient_full or test_filter_full or test_every_tensor_type_ragged_grids or test_gradient_sampled_full_size "
+           "or test_filter_sampled_radii_full_size")
     r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-x", "-q", "-k", sel], env=child,
                        capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
