@@ -12,6 +12,7 @@ struct sp_shell {
     bool grad_split_ok = false;   // the split gradient (r-theta kernel first, d/dphi GEMM with fused chain rule) is usable
     int grad_nwarps = 6, grad3_nwarps = 6, num_sms = 148;
     int grad3_ctas[2] = {0, 0};      // same for the folded kernel k_grad_rtheta3
+    int grad3_alt_nwarps = 0, grad3_alt_ctas = 0;   // narrower CTAs (4 warps) of the single-buffered k_grad_rtheta3 for small calls: more CTAs per SM, one round
     int grad_ctas[2] = {1, 0};       // resident CTAs per SM with NBUF = 1 / 2 (0: does not fit)
     size_t grad_smem[2] = {0, 0};
     int gradKT;                   // radial tiles per warp task of k_grad_rtheta2 (3 or 5)

@@ -368,9 +368,20 @@ sp_status sp_configure_kernels(sp_shell *s) {
                 if (KT == 3) { if (nb == 1) { SP_G3(3, 1) } else { SP_G3(3, 2) } }
                 else { if (nb == 1) { SP_G3(5, 1) } else { SP_G3(5, 2) } }
 #undef SP_G3
-#undef SP_G3P
                 s->grad3_ctas[nb - 1] = occ;
+                // small calls (fewer items than resident 6-warp CTAs can take in one round): 4-warp CTAs, when they split the warp
+                // tasks evenly, fit more CTAs per SM (config 5: 320 items, 3 x 148 slots instead of 2 x 148; (r,theta) 41 -> 36 us)
+                if (nb == 1 && KT == 5 && nt3 > 4 && nt3 % 4 == 0 && s->grad3_nwarps == 6 && !getenv("SP_GRAD_NWARPS") && !getenv("SP_GRAD_CTAS")) {
+                    int occ_main = occ;
+                    {
+                        const int thr = 4 * 32;
+                        if (s->PU == 44) { SP_G3P(5, 1, 44) } else { SP_G3P(5, 1, 0) }
+                    }
+                    s->grad3_alt_nwarps = 4; s->grad3_alt_ctas = occ;
+                    occ = occ_main;
+                }
                 if (const char *e = getenv("SP_GRAD_CTAS")) { const int c = atoi(e); if (c >= 1 && c < occ) s->grad3_ctas[nb - 1] = c; }   // tuning override: resident CTAs per SM
+#undef SP_G3P
             }
         }
     }
@@ -501,10 +512,18 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         const int KT = s->gradKT;
         const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
         if (s->grad3_ctas[0] > 0) {      // folded theta derivative (k_grad_rtheta3)
-            const int nthr = s->grad3_nwarps * 32;
+            int nthr = s->grad3_nwarps * 32;
             const int nb = (s->grad3_ctas[1] > 0 && p.nitems >= 3 * s->num_sms * s->grad3_ctas[1]) ? 2 : 1;
-            const int ncta = std::min(p.nitems, s->num_sms * s->grad3_ctas[nb - 1]);
+            int ncta = std::min(p.nitems, s->num_sms * s->grad3_ctas[nb - 1]);
             const size_t smb = s->grad_smem[nb - 1];
+            if (nb == 1 && s->grad3_alt_ctas > 0) {      // rounds of resident CTAs x passes of a CTA's warps over its tasks
+                const int nt3 = itiles * ((ktiles + KT - 1) / KT);
+                auto cost = [&](int ctas, int nw) { return ((p.nitems + s->num_sms * ctas - 1) / (s->num_sms * ctas)) * ((nt3 + nw - 1) / nw); };
+                if (cost(s->grad3_alt_ctas, s->grad3_alt_nwarps) < cost(s->grad3_ctas[0], s->grad3_nwarps)) {
+                    nthr = s->grad3_alt_nwarps * 32;
+                    ncta = std::min(p.nitems, s->num_sms * s->grad3_alt_ctas);
+                }
+            }
 #define SP_G3L(KT_, NB_)                                                                               \
     if (KT_ == 5 && s->PU == 44) k_grad_rtheta3<KT_, NB_, 44><<<ncta, nthr, smb, st>>>(p);             \
     else if (KT_ == 3 && s->PU == 28) k_grad_rtheta3<KT_, NB_, 28><<<ncta, nthr, smb, st>>>(p);        \
