@@ -330,7 +330,7 @@ template <int KT, int NBUF, int PUC = 0>
 __global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_rtheta3(GradParams p) {
     extern __shared__ double sm[];
     const int Nr = p.Nr, Nt = p.Nt, Np = p.Np, PU = PUC > 0 ? PUC : p.PU;
-    const int itiles = p.Nt8 >> 3, ipairs = (itiles + 1) >> 1, ktiles = p.Nr8 >> 3, kgroups = (ktiles + KT - 1) / KT;
+    const int itiles = p.Nt8 >> 3, ktiles = p.Nr8 >> 3, kgroups = (ktiles + KT - 1) / KT;
     const int NK8 = kgroups * KT * 8, n2 = 2 * Nt;
     const int prow = p.Nt8 + ((itiles & 1) ? 8 : 0);           // rows of a plane buffer
     const size_t planesz = (size_t)prow * PU;

@@ -58,7 +58,7 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp % mgroups, ng = warp / mgroups, nwarps = blockDim.x >> 5;
     const size_t vec = (size_t)Nt * Nr, dofsz = (size_t)MC4 * vec, fsz = (size_t)Nt8 * Nt8;
-    const int mca = m, mcb = L + m;                            // rows a_0..a_L, b_1..b_L
+    const int mca = m;                                         // rows a_0..a_L, then b_1..b_L (b_m = row L + m: offset offAB below)
     constexpr int TH_PKB = TH_PKB_OF(NT), TH_ARR = TH_ARR_OF(NT);
     const int stageA = NMAT * Nt8c * TH_PA, stageB = NARR * TH_ARR;
     // shared-memory slot of source array arr: the pairs a lane pair (v = 0, 1) reads together are neighbours

@@ -707,7 +707,7 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     if (!s || !u || !out || nfields < 0 || ntens < 0 || (ntens > 0 && !tens)) return SP_ERR_INVALID_ARG;
     if (!s->built) return SP_ERR_NOT_BUILT;
     cudaStream_t st = (cudaStream_t)stream;
-    const int Nr = s->Nr, Nt = s->Nt, Np = s->Np;
+    const int Nr = s->Nr, Nt = s->Nt;
     const size_t npts = s->npts, vec = (size_t)Nt * Nr;
     // ---- validate, classify, build the component list
     std::vector<int> owner(nfields, -1), types(ntens);
