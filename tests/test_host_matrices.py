@@ -61,6 +61,19 @@ def test_host_matrices_match_oracle(cfg):
     assert worst < 1e-13, worst
 
 
+@pytest.mark.parametrize("Nt,L", [(8, 6), (24, 19), (7, 4)])
+def test_filter_matrices_equatorial_reflection(Nt, L):
+    """sY_lm(pi - theta) = (-1)^(l+m) (-s)Y_lm(theta) and the Gauss grid (eq. 3) is symmetric about the equator, so with R the
+    reversal of the latitudes F^{-n}_m = R F^n_m R (F is quadratic in P, the signs cancel); F^0_m is centrosymmetric.  Holds for
+    the oracle's matrices and for the library's host build: the basis of an even/odd fold of the theta step."""
+    sh = Shell(9, Nt, 2 * Nt, 1.0, 3.0, L, host_only=True)
+    for get in (lambda n, m: oracle.filter_matrix(Nt, L, n, m), lambda n, m: sh.get_matrix(5, n, m)):
+        for n in range(0, 4):
+            for m in range(0, L + 1):
+                Fp, Fm = get(n, m), get(-n, m)
+                assert np.max(np.abs(Fm - Fp[::-1, ::-1])) < 1e-13
+
+
 def test_ghg_spatial_degree_and_layout():
     """Host logic of the GHG driver: d(u^mu) of PAPER.md:441 (g_tt 0, g_tx 1, g_xx 2; d_iab one more) and the tensor layout."""
     from paper_1104_3408_b200.ghg import ghg_tensors, spatial_degree
