@@ -406,6 +406,32 @@ class GpuWorkload:
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) / steps
 
+    def time_call_graph(self, which, steps, warmup=1):
+        """The same call alone, replayed from a CUDA graph holding one call per input copy (the headline's launch mode)."""
+        torch = self.torch
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        self.it = 0
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(self.nsets):
+                u = self.u[self.it % self.nsets]
+                self.it += 1
+                if which == "gradient":
+                    self.sh.cartesian_gradient(u, out=self.du, workspace=self.ws_g, stream=side)
+                else:
+                    self.sh.tensor_filter(u, self.cfg["tensors"], out=self.fu, workspace=self.ws_f, descs=self.descs, stream=side)
+        rounds = max(1, steps // self.nsets)
+        for _ in range(warmup):
+            g.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(rounds):
+            g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / (rounds * self.nsets)
+
     def calls_report(self, steps, peak_tf):
         """each call alone -- units/s, achieved algorithmic TFLOP/s, fraction of the FP64 peak."""
         fl = flops_per_unit(self.cfg)
@@ -417,6 +443,13 @@ class GpuWorkload:
             tf = f * self.units / (ms * 1e-3) * 1e-12
             out[which] = {"ms": ms, "value": self.units / (ms * 1e-3), "algorithmic_flops_per_unit": f, "tflops": tf,
                           "frac_of_fp64_peak": tf / peak_tf}
+            try:                                                             # same call replayed from a CUDA graph
+                msg = sorted(self.time_call_graph(which, steps) for _ in range(3))[1]
+                out[which]["graph_ms"] = msg
+                out[which]["graph_frac_of_fp64_peak"] = f * self.units / (msg * 1e-3) * 1e-12 / peak_tf
+            except Exception as ex:                                          # capture refused: the eager figure stands alone
+                out[which]["graph_ms"] = None
+                print(f"bench.py: per-call graph capture failed ({ex!r})", file=sys.stderr)
         return out
 
     def stage_times(self, reps=5):

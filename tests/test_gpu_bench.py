@@ -32,3 +32,6 @@ def test_main_arm_contract_line(extra):
     assert e["h2d_bytes_per_step"] == 50 * 33 * 48 * 96 * 8 and e["d2h_bytes_per_step"] == 4 * e["h2d_bytes_per_step"]
     assert 0.0 < e["value"] < d["value"]                   # host copies inside the timed region can only slow it down
     assert "workload" in d["config"] and "config 3" in d["config"]["workload"]
+    for which in ("gradient", "filter"):                   # each call alone: eager and replayed from a CUDA graph
+        c = d["calls"][which]
+        assert 0.0 < c["frac_of_fp64_peak"] < 1.0 and c["graph_ms"] is not None and 0.0 < c["graph_frac_of_fp64_peak"] < 1.0
