@@ -201,3 +201,143 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
 static inline size_t theta2_smem_bytes(int Nt8, bool cplx, int NT = 1) {      // NT = 1 has the larger tile; Nt8 = rows per CTA
     return (size_t)TH_STAGES * ((size_t)(cplx ? 2 : 1) * Nt8 * TH_PA + (cplx ? 4 : 2) * TH_ARR_OF(NT)) * sizeof(double);
 }
+
+// ---------------------------------------------------------------------------------------------
+// EQUATORIAL FOLD of the theta step for real components (n = 0).  The Gauss latitudes (eq. 3) are symmetric about the
+// equator and sY_lm(pi - theta) = (-1)^(l+m) (-s)Y_lm(theta), so with i' = Ntheta - 1 - i the filter matrices satisfy
+// F^{-n}_m[i'][k'] = F^n_m[i][k] (tests/test_host_matrices.py); F^0_m is centrosymmetric.  With h = Ntheta / 2 and, for k < h,
+//     xE[k] = x[k] + x[k'],   xO[k] = x[k] - x[k'],     G+-[i][k] = (F^0_m[i][k] +- F^0_m[i][k']) / 2      (h x h, built on the host)
+// the same sums regroup to   y[i] = (G+ xE)[i] + (G- xO)[i],   y[i'] = (G+ xE)[i] - (G- xO)[i]:
+// two (Ntheta/2)^2 products instead of one Ntheta^2 -- half the DMMAs, the regrouping of the two reflection folds already in
+// the path (d/dtheta: antipodal planes, Fourier transforms: phi -> 2 pi - phi).  Requires Ntheta even.
+// Data flow = the complex path of k_theta2: two matrices (G+, G-), four staged row sets (a_m top, a_m bottom reversed, b_m top,
+// b_m bottom reversed), fragments b1 = top + bottom, b2 = top - bottom, lane-local epilogue.  G: [2][L+1][h8][h8] zero padded.
+// ---------------------------------------------------------------------------------------------
+template <int MT, int NT>
+__global__ void __launch_bounds__(NT == 3 ? 384 : 896, 1)
+k_theta_fold(ThetaBatch2 comps, const double *__restrict__ G, int L, int Nt, int h8, int Nr, int MC4, int mgroups,
+             const double *__restrict__ coef, double *__restrict__ cout) {
+    extern __shared__ __align__(16) double sm[];
+    constexpr int TH_PKB = TH_PKB_OF(NT), TH_ARR = TH_ARR_OF(NT);
+    const ThetaComp2 cmp = comps.c[blockIdx.y];
+    const int m = blockIdx.x, k0 = blockIdx.z * TH_RC, h = Nt >> 1;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    const int mg = warp % mgroups, ng = warp / mgroups, nwarps = blockDim.x >> 5;
+    const size_t vec = (size_t)Nt * Nr, dofsz = (size_t)MC4 * vec, gsz = (size_t)h8 * h8;
+    const int stageA = 2 * h8 * TH_PA, stageB = 4 * TH_ARR;
+    // row sets: arr = 2 * (0: a_m, 1: b_m) + (0: top rows ascending, 1: bottom rows descending); the sets a lane pair (v = 0, 1)
+    // reads together (arr 0 and 2, arr 1 and 3) are neighbours in the NT = 1 layout
+    auto brow = [&](int arr, int r) {
+        const int slot = (arr == 0) ? 0 : (arr == 2) ? 1 : (arr == 1) ? 2 : 3;
+        return NT == 1 ? slot * TH_ARR + r * TH_PKB : (arr * TH_KC + r) * TH_PKB;
+    };
+    double *As = sm, *Bs = sm + TH_STAGES * stageA;
+    const int nrad = min(TH_RC, Nr - k0);
+    const double *G0 = G + (size_t)m * gsz;
+    const long dG = (long)(L + 1) * (long)gsz;                                  // G- relative to G+
+    const int nchunks = (h8 + TH_KC - 1) / TH_KC;
+    const int hF = tid & 7, rF0 = tid >> 3, rFstep = blockDim.x >> 3;
+    const size_t offAB = (size_t)L * vec;                                       // b_m relative to a_m
+    const double *srcA = coef + (size_t)cmp.dof * dofsz + (size_t)m * vec + k0 + lane;
+    const bool live0 = lane < nrad, live1 = lane + 32 < nrad, lane_hi = lane < TH_RC - 32;
+    auto load_chunk = [&](int kc, int st) {
+        double *as = As + st * stageA + rF0 * TH_PA + 2 * hF;
+        if (kc * TH_KC + 2 * hF < h8) {
+            const double *fs = G0 + rF0 * h8 + kc * TH_KC + 2 * hF;
+            const int fstep = rFstep * h8;
+#pragma unroll 1
+            for (int r = rF0; r < h8; r += rFstep, as += rFstep * TH_PA, fs += fstep) {
+                cp_async16(as, fs);
+                cp_async16(as + h8 * TH_PA, fs + dG);
+            }
+        } else {
+#pragma unroll 1
+            for (int r = rF0; r < h8; r += rFstep, as += rFstep * TH_PA) {
+                as[0] = 0.0; as[1] = 0.0;
+                as[h8 * TH_PA] = 0.0; as[h8 * TH_PA + 1] = 0.0;
+            }
+        }
+        const int kbase = kc * TH_KC;
+        double *bs = Bs + st * stageB + lane;
+        const int gstep = nwarps * Nr, sstep = nwarps * TH_PKB;
+#pragma unroll
+        for (int arr = 0; arr < 4; arr++) {
+            const bool bot = arr & 1;
+            const double *gp = srcA + (arr >> 1) * offAB + (size_t)(bot ? Nt - 1 - (kbase + warp) : kbase + warp) * Nr;
+            double *sp = bs + brow(arr, warp);
+            const bool arrdead = (m == 0) && (arr >> 1);                                // b_0 does not exist
+#pragma unroll 1
+            for (int r = warp; r < TH_KC; r += nwarps, sp += sstep) {
+                const bool dead = arrdead || kbase + r >= h;
+                const double *gq = dead ? srcA : gp;                                    // dead rows: any valid address (not read)
+                cp_async8_ign(sp, gq, dead || !live0);
+                if (lane_hi) cp_async8_ign(sp + 32, gq + 32, dead || !live1);
+                if (bot) gp -= gstep; else gp += gstep;
+            }
+        }
+    };
+
+    double acc[2][MT][NT][2];
+#pragma unroll
+    for (int x = 0; x < 2; x++)
+#pragma unroll
+        for (int a = 0; a < MT; a++)
+#pragma unroll
+            for (int b = 0; b < NT; b++) acc[x][a][b][0] = acc[x][a][b][1] = 0.0;
+#pragma unroll
+    for (int s = 0; s < TH_STAGES - 1; s++) {
+        if (s < nchunks) load_chunk(s, s);
+        cp_async_commit();
+    }
+    const int v = g & 1, kq = g >> 1;
+    const int oX = brow(2 * v, t), oY = brow(2 * v + 1, t);
+    for (int kc = 0; kc < nchunks; kc++) {
+        cp_async_wait<TH_STAGES - 2>();
+        __syncthreads();
+        if (kc + TH_STAGES - 1 < nchunks) load_chunk(kc + TH_STAGES - 1, (kc + TH_STAGES - 1) % TH_STAGES);
+        cp_async_commit();
+        const double *as = As + (kc % TH_STAGES) * stageA + (mg * MT * 8 + g) * TH_PA + t;
+        const double *bs = Bs + (kc % TH_STAGES) * stageB;
+#pragma unroll
+        for (int ks = 0; ks < TH_KC / 4; ks++) {
+            double b1[NT], b2[NT];
+#pragma unroll
+            for (int b = 0; b < NT; b++) {
+                const int kk = (ng * NT + b) * 4 + kq + ks * 4 * TH_PKB;
+                const double x = bs[oX + kk], y = bs[oY + kk];
+                b1[b] = x + y;
+                b2[b] = x - y;
+            }
+#pragma unroll
+            for (int a = 0; a < MT; a++) {
+                const double a1 = as[a * 8 * TH_PA + ks * 4];
+#pragma unroll
+                for (int b = 0; b < NT; b++) dmma(acc[0][a][b][0], acc[0][a][b][1], a1, b1[b]);
+                const double a2 = as[(h8 + a * 8) * TH_PA + ks * 4];
+#pragma unroll
+                for (int b = 0; b < NT; b++) dmma(acc[1][a][b][0], acc[1][a][b][1], a2, b2[b]);
+            }
+        }
+    }
+    // epilogue: lane owns the latitudes i = (mg*MT + a)*8 + g < h and i' = Ntheta - 1 - i, radius k = k0 + (ng*NT + b)*4 + t
+    double *Ro = cout + (size_t)cmp.dof * dofsz + (size_t)m * vec + k0;
+    const int eAB = (int)offAB;
+#pragma unroll
+    for (int a = 0; a < MT; a++) {
+        const int i = (mg * MT + a) * 8 + g;
+        if (i >= h) continue;
+#pragma unroll
+        for (int b = 0; b < NT; b++) {
+            const int kl = (ng * NT + b) * 4 + t;
+            if (kl >= nrad) continue;
+            const int off = i * Nr + kl, offm = (Nt - 1 - i) * Nr + kl;
+            const double p0 = acc[0][a][b][0], p1 = acc[0][a][b][1], s0 = acc[1][a][b][0], s1 = acc[1][a][b][1];
+            Ro[off] = p0 + s0;
+            Ro[offm] = p0 - s0;
+            if (m > 0) { Ro[off + eAB] = p1 + s1; Ro[offm + eAB] = p1 - s1; }
+        }
+    }
+}
+static inline size_t theta_fold_smem_bytes(int h8, int NT) {
+    return (size_t)TH_STAGES * ((size_t)2 * h8 * TH_PA + 4 * TH_ARR_OF(NT)) * sizeof(double);
+}

@@ -26,6 +26,8 @@ struct sp_shell {
     double *d_an = nullptr;        // Fourier analysis  [MC8][Np], zero padded rows    (eq. 24)
     double *d_sy = nullptr;        // Fourier synthesis [J8][MC4], zero padded         (eq. 23)
     double *d_F = nullptr;         // F^n_m [7][L+1][Nt8][Nt4], zero padded            (eq. 62)
+    double *d_G = nullptr;         // equatorial fold of F^0_m: G+, G- [2][L+1][h8][h8], zero padded (Ntheta even; k_theta_fold)
+    int h8 = 0;                    // Ntheta / 2 rounded up to 8
     // shared-memory-staged phi GEMM operands: rows padded to the warp tiling, K padded to 8, zero filled
     double *d_fd3p = nullptr;
     int fd3_MT = 0, fd3_mg = 0, fd3_Mpad = 0;

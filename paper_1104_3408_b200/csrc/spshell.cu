@@ -64,7 +64,7 @@ extern "C" sp_status sp_shell_create(int Nr, int Nt, int Np, double rin, double 
 }
 
 static void free_dev(sp_shell *s) {
-    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_fd3p, &s->d_gm, &s->d_gp, &s->m_ac.d, &s->m_as.d, &s->m_sc.d, &s->m_ss.d, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
+    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_G, &s->d_fd3p, &s->d_gm, &s->d_gp, &s->m_ac.d, &s->m_as.d, &s->m_sc.d, &s->m_ss.d, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
                     &s->d_inv_sin_t, &s->d_sin_p, &s->d_cos_p};
     for (auto q : p) {
         if (*q) cudaFree(*q);
@@ -130,6 +130,22 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
                 for (int j = 0; j < Nt; j++)
                     f[((size_t)q * s->Nt8 + i) * s->Nt8 + j] = H.F[((size_t)q * Nt + i) * Nt + j];
         if ((st = upload(&s->d_F, f.data(), f.size())) != SP_OK) return st;
+    }
+    s->h8 = 0;
+    if (Nt % 2 == 0) {   // equatorial fold of F^0_m (k_theta_fold): G+- [i][k] = (F[i][k] +- F[i][Nt-1-k]) / 2, i, k < Nt / 2
+        const int h = Nt / 2, h8 = (h + 7) / 8 * 8;
+        std::vector<double> gf((size_t)2 * (L + 1) * h8 * h8, 0.0);
+        for (int m = 0; m <= L; m++) {
+            const double *F0 = H.F.data() + ((size_t)(3 * (L + 1) + m) * Nt) * Nt;
+            for (int i = 0; i < h; i++)
+                for (int k = 0; k < h; k++) {
+                    const double a = F0[(size_t)i * Nt + k], b = F0[(size_t)i * Nt + (Nt - 1 - k)];
+                    gf[(((size_t)m) * h8 + i) * h8 + k] = 0.5 * (a + b);
+                    gf[(((size_t)(L + 1) + m) * h8 + i) * h8 + k] = 0.5 * (a - b);
+                }
+        }
+        if ((st = upload(&s->d_G, gf.data(), gf.size())) != SP_OK) return st;
+        s->h8 = h8;
     }
     {   // padded operands of k_phi_gemm: FD_{Np}, and the folded Fourier blocks (entries taken from H.an / H.sy)
         PhiTiling t1 = phi_tiling(Np);
@@ -276,9 +292,35 @@ static sp_status launch_theta2(const sp_shell *s, int v, const std::vector<Theta
     if (fork) {
         if (cudaEventRecord(s->ev_fork, main_st) != cudaSuccess || cudaStreamWaitEvent(s->aux, s->ev_fork, 0) != cudaSuccess) return SP_ERR_CUDA;
     }
+    // real components: equatorially folded kernel (half the DMMAs) when Ntheta is even; SP_THETA_FOLD=0 switches it off (experiments)
+    static const bool fold_env = [] { const char *e = getenv("SP_THETA_FOLD"); return !e || atoi(e) != 0; }();
+    int fMT = 0, fmg = 0;
+    if (s->d_G && fold_env) {
+        const int mt = s->h8 / 8;
+        fMT = (mt % 3 == 0) ? 3 : (mt % 4 == 0) ? 4 : (mt < 3 ? mt : (mt % 2 == 0 ? 2 : 1));
+        fmg = mt / fMT;
+        if (fmg * (9 / NT) > (NT == 3 ? 12 : 28) || theta_fold_smem_bytes(s->h8, NT) > 227 * 1024) fMT = 0;
+    }
     for (int pass = 1; pass >= 0; pass--) {
         const std::vector<ThetaComp2> &lst = pass ? cx : rl;
         st = (fork && pass == 0) ? s->aux : main_st;
+        if (pass == 0 && fMT > 0) {
+            const size_t smf = theta_fold_smem_bytes(s->h8, NT);
+            const dim3 fblock(fmg * (9 / NT) * 32);
+            for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
+                ThetaBatch2 b;
+                const int nb = (int)std::min<size_t>(SP_THETA2_BATCH, lst.size() - c0);
+                for (int q = 0; q < nb; q++) b.c[q] = lst[c0 + q];
+                const dim3 grid(s->L + 1, nb, gz);
+#define SP_THF(MTV, NTV) k_theta_fold<MTV, NTV><<<grid, fblock, smf, st>>>(b, s->d_G, s->L, s->Nt, s->h8, s->Nr, s->MC4, fmg, coef1, coef2);
+#define SP_THFM(NTV) switch (fMT) { case 1: SP_THF(1, NTV) break; case 2: SP_THF(2, NTV) break; case 3: SP_THF(3, NTV) break; default: SP_THF(4, NTV) break; }
+                if (NT == 3) { SP_THFM(3) } else { SP_THFM(1) }
+#undef SP_THFM
+#undef SP_THF
+                g_sp_launches += 1;
+            }
+            continue;
+        }
         const size_t sm = theta2_smem_bytes(s->Nt8 / rsplit, pass == 1, NT);
         for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
             ThetaBatch2 b;
@@ -421,6 +463,14 @@ sp_status sp_configure_kernels(sp_shell *s) {
     SP_CUDA(cudaFuncSetAttribute(k_theta2<MTV, NTV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
         SP_TA(1, 3) SP_TA(2, 3) SP_TA(3, 3) SP_TA(4, 3) SP_TA(1, 1) SP_TA(2, 1) SP_TA(3, 1) SP_TA(4, 1)
 #undef SP_TA
+        if (s->d_G) {
+            const int tf3 = (int)theta_fold_smem_bytes(s->h8, 3), tf1 = (int)theta_fold_smem_bytes(s->h8, 1);
+#define SP_TF(MTV)                                                                                                      \
+    if (tf3 <= 227 * 1024) SP_CUDA(cudaFuncSetAttribute(k_theta_fold<MTV, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tf3)); \
+    if (tf1 <= 227 * 1024) SP_CUDA(cudaFuncSetAttribute(k_theta_fold<MTV, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tf1));
+            SP_TF(1) SP_TF(2) SP_TF(3) SP_TF(4)
+#undef SP_TF
+        }
         // measure, don't guess: time the candidate variants (warp tilings NT = 3 / 1, without and with the row-block split: codes 3, 1,
         // 23, 21) on scratch data shaped like a GHG state (12 real + 18 complex components = 48 coefficient arrays), keep the winner
         const int cand[4] = {3, 1, 23, 21};

@@ -298,7 +298,7 @@ def test_shell_too_large_for_the_plane_kernels_is_refused_and_extreme_small_shel
 @pytest.mark.parametrize("env", [
     {"SP_THETA_NT": "1", "SP_GRAD_NWARPS": "2", "SP_GRAD_CTAS": "1", "SP_DPHI_FOLD_MIN": "16", "SP_PHI_NC": "32"},
     {"SP_THETA_NT": "3", "SP_GRAD_KT": "3", "SP_GRAD_NWARPS": "4", "SP_PHI_NC": "64", "SP_PHI_MSPLIT": "1"},
-    {"SP_THETA_NT": "23"},
+    {"SP_THETA_NT": "23", "SP_THETA_FOLD": "0"},
     {"SP_THETA_NT": "21", "SP_PHI_MSPLIT": "2"},
 ])
 def test_tuning_overrides_keep_parity(env):
