@@ -65,7 +65,8 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     auto slot = [](int arr) { return CPLX ? ((arr == 0) ? 0 : (arr == 2) ? 1 : (arr == 3) ? 2 : 3) : arr; };
     // offset of (array, row) in a stage of the coefficient tile
     auto brow = [&](int arr, int r) { return NT == 1 ? slot(arr) * TH_ARR + r * TH_PKB : (arr * TH_KC + r) * TH_PKB; };
-    double *As = sm, *Bs = sm + TH_STAGES * stageA;
+    // only min(TH_STAGES, K chunks) stages are allocated (theta2_smem_bytes): short K leaves room for more CTAs per SM
+    double *As = sm, *Bs = sm + min(TH_STAGES, (Nt8 + TH_KC - 1) / TH_KC) * stageA;
     const int nrad = min(TH_RC, Nr - k0);
     // source arrays: real: [a_m, b_m]; complex: [a^r, b^r, a^i, b^i]
     const double *srcR = coef + (size_t)cmp.dof * dofsz + k0;            // arr = 2*part + (0: a_m, 1: b_m)
@@ -198,8 +199,8 @@ k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt
     }
 }
 
-static inline size_t theta2_smem_bytes(int Nt8, bool cplx, int NT = 1) {      // NT = 1 has the larger tile; Nt8 = rows per CTA
-    return (size_t)TH_STAGES * ((size_t)(cplx ? 2 : 1) * Nt8 * TH_PA + (cplx ? 4 : 2) * TH_ARR_OF(NT)) * sizeof(double);
+static inline size_t theta2_smem_bytes(int Nt8, bool cplx, int NT = 1, int kdim = 1 << 20) {      // NT = 1 has the larger tile; Nt8 = rows per CTA, kdim = padded K
+    return (size_t)std::min(TH_STAGES, (kdim + TH_KC - 1) / TH_KC) * ((size_t)(cplx ? 2 : 1) * Nt8 * TH_PA + (cplx ? 4 : 2) * TH_ARR_OF(NT)) * sizeof(double);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -231,7 +232,7 @@ k_theta_fold(ThetaBatch2 comps, const double *__restrict__ G, int L, int Nt, int
         const int slot = (arr == 0) ? 0 : (arr == 2) ? 1 : (arr == 1) ? 2 : 3;
         return NT == 1 ? slot * TH_ARR + r * TH_PKB : (arr * TH_KC + r) * TH_PKB;
     };
-    double *As = sm, *Bs = sm + TH_STAGES * stageA;
+    double *As = sm, *Bs = sm + min(TH_STAGES, (h8 + TH_KC - 1) / TH_KC) * stageA;
     const int nrad = min(TH_RC, Nr - k0);
     const double *G0 = G + (size_t)m * gsz;
     const long dG = (long)(L + 1) * (long)gsz;                                  // G- relative to G+
@@ -339,5 +340,5 @@ k_theta_fold(ThetaBatch2 comps, const double *__restrict__ G, int L, int Nt, int
     }
 }
 static inline size_t theta_fold_smem_bytes(int h8, int NT) {
-    return (size_t)TH_STAGES * ((size_t)2 * h8 * TH_PA + 4 * TH_ARR_OF(NT)) * sizeof(double);
+    return (size_t)std::min(TH_STAGES, (h8 + TH_KC - 1) / TH_KC) * ((size_t)2 * h8 * TH_PA + 4 * TH_ARR_OF(NT)) * sizeof(double);
 }

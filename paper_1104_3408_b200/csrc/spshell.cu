@@ -276,7 +276,7 @@ static bool theta2_fits(const sp_shell *s, int v) {
     if ((s->Nt8 / 8) % rs != 0 || s->Nt8 / rs < 8) return false;
     int MT, mg;
     theta2_tiling(s, v, MT, mg);
-    return mg * (9 / NT) <= (NT == 3 ? 12 : 28) && theta2_smem_bytes(s->Nt8 / rs, true, NT) <= 227 * 1024;      // launch bounds of k_theta2
+    return mg * (9 / NT) <= (NT == 3 ? 12 : 28) && theta2_smem_bytes(s->Nt8 / rs, true, NT, s->Nt8) <= 227 * 1024;      // launch bounds of k_theta2
 }
 static sp_status launch_theta2(const sp_shell *s, int v, const std::vector<ThetaComp2> &rl, const std::vector<ThetaComp2> &cx,
                                const double *coef1, double *coef2, cudaStream_t st) {
@@ -321,7 +321,7 @@ static sp_status launch_theta2(const sp_shell *s, int v, const std::vector<Theta
             }
             continue;
         }
-        const size_t sm = theta2_smem_bytes(s->Nt8 / rsplit, pass == 1, NT);
+        const size_t sm = theta2_smem_bytes(s->Nt8 / rsplit, pass == 1, NT, s->Nt8);
         for (size_t c0 = 0; c0 < lst.size(); c0 += SP_THETA2_BATCH) {
             ThetaBatch2 b;
             const int nb = (int)std::min<size_t>(SP_THETA2_BATCH, lst.size() - c0);
