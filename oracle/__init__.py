@@ -197,18 +197,21 @@ def wave_dt(Nr, Nt, Np, rmin, rmax, lam=4.0):
     return lam * min(r[1] - r[0], dphi)
 
 
-def wave_rk4(u, Nr, Nt, Np, rmin, rmax, L, tensors, dt, nsteps):
+def wave_rk4(u, Nr, Nt, Np, rmin, rmax, L, tensors, dt, nsteps, on_step=None):
     """Classical RK4 with the Yn filter applied to the initial data, to every stage
-    state before its RHS and to the final combination: 4 filters per step (reading W5)."""
+    state before its RHS and to the final combination: 4 filters per step (reading W5).
+    on_step(step, u), if given, is called after every completed step (observation only: snapshots of a long run)."""
     F = lambda v: tensor_filter(v, Nr, Nt, Np, L, tensors)
     R = lambda v: wave_rhs(v, Nr, Nt, Np, rmin, rmax)
     u = F(np.array(u, dtype=np.float64))
-    for _ in range(nsteps):
+    for step in range(1, nsteps + 1):
         k1 = R(u)
         k2 = R(F(u + 0.5 * dt * k1))
         k3 = R(F(u + 0.5 * dt * k2))
         k4 = R(F(u + dt * k3))
         u = F(u + dt / 6.0 * (k1 + 2.0 * k2 + 2.0 * k3 + k4))
+        if on_step is not None:
+            on_step(step, u)
     return u
 
 

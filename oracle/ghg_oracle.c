@@ -23,11 +23,16 @@
  * Pins (tests/test_oracle_ghg.py): the Kerr-Schild metric (A.17) is a static solution of the
  * Einstein equations, so the RHS of data built from it -- for the centred hole and for a hole
  * displaced from the origin, which breaks every symmetry of the grid -- must vanish to the
- * truncation error of the spectral derivatives and fall exponentially with Nr (any dropped term,
- * wrong sign or misplaced index leaves an O(1) residual that does not converge); Minkowski gives
- * exactly zero; alpha, beta^i, gamma^{ij} against the closed forms (A.19); with the boundary
- * condition on, the incoming characteristic combinations of (A.14) vanish and the outgoing one
- * and d_t g_ab are those of the unconstrained RHS.
+ * truncation error of the spectral derivatives and fall exponentially with Nr (a dropped term,
+ * wrong sign or misplaced index in any term that does NOT vanish on constraint-satisfying data
+ * leaves an O(1) residual that does not converge); Minkowski gives exactly zero; alpha, beta^i,
+ * gamma^{ij} against the closed forms (A.19); with the boundary condition on, the incoming
+ * characteristic combinations of (A.14) vanish and the outgoing one and d_t g_ab are those of
+ * the unconstrained RHS.  The terms proportional to the constraints d_i g_ab - d_iab and
+ * H_a + Gamma_a (+alpha d_i g_ab, -alpha d_iab in (A.9); -beta^k d_k g_ab, +beta^i d_iab and the
+ * gamma0 term in (A.10)) are silent on that data; they are pinned one by one through the closed-form
+ * linear response on a flat background (Minkowski and Minkowski in shifted coordinates), each
+ * test checked to fail when the sign of its term is flipped.
  */
 #include <math.h>
 #include <stdlib.h>

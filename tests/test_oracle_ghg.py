@@ -134,3 +134,163 @@ def test_characteristic_speeds_printed_in_the_paper():
         v = -alpha - s_dn @ beta_up
         assert abs(v - printed) < 0.006, (rmin, v)
         assert abs((alpha - s_dn @ beta_up)) < 1e-12 if rmin == 2.00 else True      # the outgoing speed vanishes on the horizon
+
+
+# ---- the terms proportional to the constraints C_iab = d_i g_ab - d_iab and C_a = H_a + Gamma_a --------------------------
+# They vanish identically on the constraint-satisfying static data above, so they get their own pins: the LINEAR RESPONSE of
+# the printed equations (A.9), (A.10) on a flat background to ONE small perturbation at a time has a closed form.  The
+# response is taken by a central difference in eps (even orders cancel), the oracle receives the "numerical derivatives" du
+# as an argument, so every derivative slot can be driven independently.  Backgrounds: Minkowski (alpha = 1, beta = 0,
+# n^a = (1,0,0,0), n_a = (-1,0,0,0)) and Minkowski in Galilean-shifted coordinates x' = x + b t (a constant metric
+# g_tt = -1 + b.b, g_ti = b_i, g_ij = delta_ij: alpha = 1, beta^i = b_i, gamma^ij = delta^ij, Gamma = 0).
+_SYM = [[0, 1, 2, 3], [1, 4, 5, 6], [2, 5, 7, 8], [3, 6, 8, 9]]
+_G = (3, 2, 4)            # Nr, Nt, Np: the RHS is pointwise
+
+
+def _flat_state(b=(0.0, 0.0, 0.0)):
+    Nr, Nt, Np = _G
+    b = np.asarray(b, dtype=float)
+    g4 = np.diag([-1.0, 1.0, 1.0, 1.0])
+    g4[0, 0] += b @ b
+    g4[0, 1:] = g4[1:, 0] = b
+    u = np.zeros((50, Np, Nt, Nr))
+    for a in range(4):
+        for c in range(a, 4):
+            u[_SYM[a][c]] = g4[a, c]
+    return u, g4
+
+
+def _sym_field(rng, lead=()):
+    """random [*lead, 4, 4, Np, Nt, Nr], symmetric in the two 4-indices"""
+    Nr, Nt, Np = _G
+    s = rng.standard_normal(tuple(lead) + (4, 4, Np, Nt, Nr))
+    return s + np.swapaxes(s, len(lead), len(lead) + 1)
+
+
+def _response(make, eps=1e-6):
+    """(rhs(+eps) - rhs(-eps)) / (2 eps) of oracle.ghg_rhs; make(eps) -> (u, du, H, dH).  Returns tg [4,4,..], tk, td [3,4,4,..]."""
+    Nr, Nt, Np = _G
+    r = [oracle.ghg_rhs(*make(e), Nr, Nt, Np, 1.0, 2.0) for e in (eps, -eps)]
+    d = (r[0] - r[1]) / (2 * eps)
+    full = lambda base: np.array([[d[base + _SYM[a][c]] for c in range(4)] for a in range(4)])
+    return full(0), full(10), np.array([full(20 + 10 * i) for i in range(3)])
+
+
+def _put(u, base, s):
+    for a in range(4):
+        for c in range(a, 4):
+            u[base + _SYM[a][c]] += s[a, c]
+
+
+def test_A9_minus_alpha_d_iab_term():
+    """Minkowski, d_iab = eps c_iab, everything else zero: (A.9) reduces to d_t d_iab = -eps c_iab (the -alpha d_iab term;
+    the n n d k and gamma n d d terms are second order, every derivative slot is zero)."""
+    rng = np.random.default_rng(21)
+    c = _sym_field(rng, (3,))
+    Nr, Nt, Np = _G
+
+    def make(e):
+        u, _ = _flat_state()
+        for i in range(3):
+            _put(u, 20 + 10 * i, e * c[i])
+        return u, np.zeros((3, 50, Np, Nt, Nr)), np.zeros((4, Np, Nt, Nr)), np.zeros((3, 4, Np, Nt, Nr))
+
+    tg, tk, td = _response(make)
+    assert np.abs(td + c).max() < 1e-8
+    assert np.abs(tg).max() < 1e-8                      # (A.8): beta = 0, k = 0
+
+
+def test_A9_plus_alpha_di_g_ab_term():
+    """Minkowski + eps h_ab with the derivative slot of g_ab driven by eps s_iab, d = k = 0: (A.9) gives d_t d_iab = +eps s_iab
+    (the +alpha d_i g_ab term) and (A.10) nothing at first order (its -beta^k d_k g_ab is second order here)."""
+    rng = np.random.default_rng(22)
+    h, s = _sym_field(rng), _sym_field(rng, (3,))
+    Nr, Nt, Np = _G
+
+    def make(e):
+        u, _ = _flat_state()
+        _put(u, 0, e * h)
+        du = np.zeros((3, 50, Np, Nt, Nr))
+        for i in range(3):
+            _put(du[i], 0, e * s[i])
+        return u, du, np.zeros((4, Np, Nt, Nr)), np.zeros((3, 4, Np, Nt, Nr))
+
+    tg, tk, td = _response(make)
+    assert np.abs(td - s).max() < 1e-8
+    assert np.abs(tk).max() < 1e-8
+
+
+def test_A10_gamma0_constraint_damping_term():
+    """Minkowski, H_a = eps w_a (no derivative), everything else zero: Gamma_a = 0, nabla_(a H_b) = 0 at first order, so (A.10)
+    reduces to d_t k_ab = gamma0 alpha (2 delta^c_(a n_b) - g_ab n^c)(H_c + Gamma_c) = eps (n_b w_a + n_a w_b - eta_ab n^c w_c)
+    with n_a = (-1,0,0,0), n^a = (1,0,0,0), gamma0 = 1 (PAPER.md:662, 674-678)."""
+    rng = np.random.default_rng(23)
+    Nr, Nt, Np = _G
+    w = rng.standard_normal((4, Np, Nt, Nr))
+    eta = np.diag([-1.0, 1.0, 1.0, 1.0])
+    n_dn, n_up = np.array([-1.0, 0, 0, 0]), np.array([1.0, 0, 0, 0])
+
+    def make(e):
+        u, _ = _flat_state()
+        return u, np.zeros((3, 50, Np, Nt, Nr)), e * w, np.zeros((3, 4, Np, Nt, Nr))
+
+    tg, tk, td = _response(make)
+    nw = np.einsum("c,c...->...", n_up, w)
+    want = np.einsum("b,a...->ab...", n_dn, w) + np.einsum("a,b...->ab...", n_dn, w) - eta[:, :, None, None, None] * nw
+    assert np.abs(tk - want).max() < 1e-8
+    assert np.abs(td).max() < 1e-8 and np.abs(tg).max() < 1e-8
+
+
+def test_A10_minus_beta_dk_g_ab_term():
+    """Shifted flat background (beta^i = b_i), derivative slot of g_ab driven by eps s_kab, d = k = 0: the only first-order
+    terms are d_t d_iab = alpha s_iab and, in (A.10), -beta^k d_k g_ab = -eps b^k s_kab."""
+    rng = np.random.default_rng(24)
+    b = np.array([0.3, -0.2, 0.25])
+    s = _sym_field(rng, (3,))
+    Nr, Nt, Np = _G
+
+    def make(e):
+        u, _ = _flat_state(b)
+        du = np.zeros((3, 50, Np, Nt, Nr))
+        for i in range(3):
+            _put(du[i], 0, e * s[i])
+        return u, du, np.zeros((4, Np, Nt, Nr)), np.zeros((3, 4, Np, Nt, Nr))
+
+    tg, tk, td = _response(make)
+    assert np.abs(tk + np.einsum("k,k...->...", b, s)).max() < 1e-8
+    assert np.abs(td - s).max() < 1e-8
+
+
+def test_A10_plus_beta_d_iab_term_and_A8():
+    """Shifted flat background, d_iab = eps v_i w_ab with w_ab trace-free and orthogonal to V_a = (b.v, v_i) (built with numpy
+    from the constant 4-metric): then D_a g_bc = eps V_a w_bc gives Gamma_c = eps (V^b w_bc - V_c tr w / 2) = 0, so the
+    constraint-damping term is silent and (A.10) reduces to its last term, d_t k_ab = +beta^i d_iab = eps (b.v) w_ab;
+    (A.8) gives the same for d_t g_ab, (A.9) gives -alpha d_iab."""
+    rng = np.random.default_rng(25)
+    b = np.array([0.3, -0.2, 0.25])
+    v = np.array([0.7, 0.4, -0.5])
+    _, g4 = _flat_state(b)
+    gi = np.linalg.inv(g4)
+    V_dn = np.concatenate([[b @ v], v])
+    V_up = gi @ V_dn
+    VV = V_dn @ V_up
+    assert abs(VV) > 0.1
+    Pi = np.eye(4) - np.outer(V_up, V_dn) / VV                  # Pi^c_a: projects orthogonally to V
+    S = rng.standard_normal((4, 4)); S = S + S.T
+    w = Pi.T @ S @ Pi
+    hproj = g4 - np.outer(V_dn, V_dn) / VV
+    w = w - np.einsum("ab,ab->", gi, w) / 3.0 * hproj
+    assert np.abs(w @ V_up).max() < 1e-13 and abs(np.einsum("ab,ab->", gi, w)) < 1e-13 and np.abs(w).max() > 0.1
+    Nr, Nt, Np = _G
+    wf = w[:, :, None, None, None] * np.ones((Np, Nt, Nr))
+
+    def make(e):
+        u, _ = _flat_state(b)
+        for i in range(3):
+            _put(u, 20 + 10 * i, e * v[i] * wf)
+        return u, np.zeros((3, 50, Np, Nt, Nr)), np.zeros((4, Np, Nt, Nr)), np.zeros((3, 4, Np, Nt, Nr))
+
+    tg, tk, td = _response(make)
+    assert np.abs(tk - (b @ v) * wf).max() < 1e-8
+    assert np.abs(tg - (b @ v) * wf).max() < 1e-8
+    assert np.abs(td + v[:, None, None, None, None, None] * wf[None]).max() < 1e-8

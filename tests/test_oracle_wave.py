@@ -69,3 +69,46 @@ def test_short_evolution_tracks_exact_solution():
     ex = synth.wave_exact(c, n * dt, amps=(1.0, 0.8, -0.6))
     assert np.max(np.abs(u - ex)) < 2e-2 * np.max(np.abs(ex))
     assert np.max(np.abs(u - u0)) > 10 * np.max(np.abs(u - ex))                       # it actually moved
+
+
+# ---- oracle.wave_rk4 is "standard fourth order Runge-Kutta": order and exact one-step amplification ------------
+# With an empty tensor list oracle.tensor_filter copies every field through, so wave_rk4 is the bare time integrator of the
+# LINEAR system du/dt = A u, A = oracle.wave_rhs (gradient + characteristic boundary condition).
+def _rk4_nofilter(u0, c, dt, n):
+    return oracle.wave_rk4(u0, c["Nr"], c["Nt"], c["Np"], c["rmin"], c["rmax"], c["L"], [], dt, n)
+
+
+def test_rk4_one_step_is_the_degree_4_taylor_polynomial_of_the_linear_system():
+    """For a linear autonomous system one step of any 4-stage 4th-order Runge-Kutta method is
+    u(dt) = (1 + z + z^2/2 + z^3/6 + z^4/24) u(0), z = dt A.  Euler, RK2, or stage weights 1/4,1/4,1/4,1/4 all give a
+    different polynomial.  A is applied through oracle.wave_rhs (white-noise data: every mode, both boundaries)."""
+    c = _cfg(9, 6)
+    Nr, Nt, Np = c["Nr"], c["Nt"], c["Np"]
+    u0 = np.random.default_rng(8).standard_normal((5, Np, Nt, Nr))
+    dt = 0.7 * oracle.wave_dt(Nr, Nt, Np, c["rmin"], c["rmax"])
+    A = lambda v: oracle.wave_rhs(v, Nr, Nt, Np, c["rmin"], c["rmax"])
+    term, want = u0.copy(), u0.copy()
+    for q in (1, 2, 3, 4):
+        term = dt / q * A(term)
+        want += term
+    got = _rk4_nofilter(u0, c, dt, 1)
+    scale = np.max(np.abs(want))
+    assert np.max(np.abs(got - want)) < 1e-13 * scale
+    # discriminating power: the z^4/24 and z^3/6 terms are far above the tolerance
+    assert np.max(np.abs(term)) > 1e-4 * scale
+    # two steps compose
+    assert np.max(np.abs(_rk4_nofilter(u0, c, dt, 2) - _rk4_nofilter(got, c, dt, 1))) < 1e-13 * scale
+
+
+def test_rk4_converges_with_fourth_order():
+    """Same data to the same final time with dt and dt/2 against a dt/8 reference: the error ratio is 2^4 = 16 (+- 20 %)."""
+    c = _cfg(13, 8)
+    Nr, Nt, Np = c["Nr"], c["Nt"], c["Np"]
+    u0 = synth.wave_exact(c, 0.0, amps=(1.0, 0.8, -0.6))
+    dt = 0.5 * oracle.wave_dt(Nr, Nt, Np, c["rmin"], c["rmax"])       # unfiltered, the default lambda = 4 is unstable on this grid
+    n = 8
+    ref = _rk4_nofilter(u0, c, dt / 8, 8 * n)
+    e1 = np.max(np.abs(_rk4_nofilter(u0, c, dt, n) - ref))
+    e2 = np.max(np.abs(_rk4_nofilter(u0, c, dt / 2, 2 * n) - ref))
+    assert e2 > 1e-11 * np.max(np.abs(ref))              # well above round-off
+    assert 0.8 * 16 < e1 / e2 < 1.2 * 16, e1 / e2
