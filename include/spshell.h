@@ -130,6 +130,12 @@ sp_status sp_rhs_ghg(const sp_shell *shell, const double *u_dev, const double *H
  * 20..49); fills k_ab = (beta^i/alpha) d_iab (A.6) into fields 10..19 and H_a = -Gamma_a (A.18) into H (4 fields). */
 sp_status sp_ghg_init(const sp_shell *shell, double *u_dev, double *H_dev, void *cuda_stream);
 
+/* Time step of the method of lines, eq. (63) (reading W4): dt = lambda * min(dx) with min(dx) the
+ * smaller of the first radial spacing r_1 - r_0 and the azimuthal spacing 2 r_0 sin(theta_0) sin(pi / Nphi) on the innermost
+ * sphere next to the pole.  Host arithmetic on the shell's grid parameters; no device, no build needed.  lambda <= 0 is
+ * SP_ERR_INVALID_ARG. */
+sp_status sp_wave_dt(const sp_shell *shell, double lambda, double *dt_out);
+
 /* y <- a*x + b*y over n doubles (the RK4 combination steps of config 5). */
 sp_status sp_axpby(double a, const double *x_dev, double b, double *y_dev, size_t n, void *cuda_stream);
 

@@ -8,7 +8,7 @@ _lib = None
 # every symbol include/spshell.h declares
 EXPORTED_SYMBOLS = [
     "sp_shell_create", "sp_shell_destroy", "sp_build_matrices", "sp_workspace_bytes", "sp_cartesian_gradient",
-    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_axpby", "sp_rk4_stage", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
+    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_wave_dt", "sp_axpby", "sp_rk4_stage", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
     "sp_status_string", "sp_profile_enable", "sp_profile_read", "sp_launch_count",
 ]
 
@@ -44,6 +44,7 @@ def lib():
         L.sp_tensor_filter.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(_TensorDesc), C.c_int,
                                        C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rhs_first_order_wave.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sp_wave_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.sp_axpby.argtypes = [C.c_double, C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rk4_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_size_t,
                                    C.c_void_p]
@@ -216,6 +217,12 @@ class Shell:
         _check(lib().sp_rhs_first_order_wave(self._h, u.data_ptr(), out.data_ptr(), ws.data_ptr(), ws.numel() * 8,
                                              _stream_ptr(stream)), "sp_rhs_first_order_wave")
         return out
+
+    def wave_dt(self, lam=4.0):
+        """dt = lambda * min(dx), eq. 63 (sp_wave_dt)."""
+        v = C.c_double()
+        _check(lib().sp_wave_dt(self._h, float(lam), C.byref(v)), "sp_wave_dt")
+        return v.value
 
     def ghg_workspace_bytes(self):
         n = C.c_size_t()

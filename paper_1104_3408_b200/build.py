@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libspshell.so")
 SOURCES = ["spshell.cu", "host_build.cpp", "sp_device.cuh", "sp_internal.h", "kernels_gemm.cuh", "kernels_gemm2.cuh", "kernels_gradphi.cuh", "kernels_theta2.cuh", "kernels_grad.cuh",
-           "kernels_filter.cuh", "kernels_wave.cuh", "kernels_ghg.cuh"]
+           "kernels_filter.cuh", "kernels_fused.cuh", "kernels_wave.cuh", "kernels_ghg.cuh"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 

@@ -40,6 +40,10 @@ struct sp_shell {
     bool gf_ok = false;
     int theta_NT = 0;             // k_theta2 variant chosen at build time: NT + 20 * (rsplit - 1), NT = 3 or 1 column tiles per warp, rsplit = 1 or 2 row blocks (3, 1, 23, 21; 0: generic kernel)
     PhiMat m_ac, m_as, m_sc, m_ss;   // analysis cos [L+1][J/2+1], sin [L][J/2-1]; synthesis cos [J/2+1][L+1], sin [J/2-1][L]
+    // operands of the fused filter kernels (kernels_fused.cuh), zero padded: analysis Ac [f_Mp][f_ldc] (a_0..a_L over jj = 0..h),
+    // As [f_Mp][f_lds] (b_1..b_L over q, jj = h-1-q); synthesis Sc, Ss [f_Jp][f_ldk] (rows jj = 0..h; Ss rows 0 and h are zero)
+    double *d_fAc = nullptr, *d_fAs = nullptr, *d_fSc = nullptr, *d_fSs = nullptr;
+    int f_Mp = 0, f_ldc = 0, f_lds = 0, f_Jp = 0, f_ldk = 0;
     double *d_inv_r = nullptr, *d_sin_t = nullptr, *d_cos_t = nullptr, *d_inv_sin_t = nullptr, *d_sin_p = nullptr,
            *d_cos_p = nullptr;     // Jacobian / triad factors                          (eq. 6, 51)
     // optional per-stage timing (sp_profile_enable): events recorded on the caller's stream

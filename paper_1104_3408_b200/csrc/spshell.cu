@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 #include <cstdint>
 
+#include <cmath>
 #include <cstdio>
 #include <algorithm>
 #include <cstring>
@@ -64,7 +65,7 @@ extern "C" sp_status sp_shell_create(int Nr, int Nt, int Np, double rin, double 
 }
 
 static void free_dev(sp_shell *s) {
-    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_G, &s->d_fd3p, &s->d_gm, &s->d_gp, &s->m_ac.d, &s->m_as.d, &s->m_sc.d, &s->m_ss.d, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
+    double **p[] = {&s->d_cd, &s->d_g2, &s->d_g3, &s->d_an, &s->d_sy, &s->d_F, &s->d_G, &s->d_fd3p, &s->d_gm, &s->d_gp, &s->m_ac.d, &s->m_as.d, &s->m_sc.d, &s->m_ss.d, &s->d_fAc, &s->d_fAs, &s->d_fSc, &s->d_fSs, &s->d_inv_r, &s->d_sin_t, &s->d_cos_t,
                     &s->d_inv_sin_t, &s->d_sin_p, &s->d_cos_p};
     for (auto q : p) {
         if (*q) cudaFree(*q);
@@ -183,6 +184,26 @@ extern "C" sp_status sp_build_matrices(sp_shell *s) {
         if ((st = mk(s->m_as, L, h - 1, [&](int r, int c) { return H.an[(size_t)(2 * (r + 1)) * Np + (c + 1)]; })) != SP_OK) return st;
         if ((st = mk(s->m_sc, h + 1, L + 1, [&](int j, int m) { return H.sy[(size_t)j * MC + (m == 0 ? 0 : 2 * m - 1)]; })) != SP_OK) return st;
         if ((st = mk(s->m_ss, h - 1, L, [&](int r, int c) { return H.sy[(size_t)(r + 1) * MC + 2 * (c + 1)]; })) != SP_OK) return st;
+        {   // operands of the fused kernels (kernels_fused.cuh): same entries, their own padding
+            s->f_Mp = round_up(L + 1, 8); s->f_ldc = round_up(h + 1, 16); s->f_lds = round_up(std::max(h - 1, 1), 16);
+            s->f_Jp = round_up(h + 1, 8); s->f_ldk = round_up(L + 1, 16);
+            std::vector<double> ac((size_t)s->f_Mp * s->f_ldc, 0.0), as((size_t)s->f_Mp * s->f_lds, 0.0);
+            std::vector<double> sc((size_t)s->f_Jp * s->f_ldk, 0.0), ss(sc.size(), 0.0);
+            for (int m = 0; m <= L; m++)
+                for (int jj = 0; jj <= h; jj++) {
+                    ac[(size_t)m * s->f_ldc + jj] = H.an[(size_t)(m == 0 ? 0 : 2 * m - 1) * Np + jj];
+                    sc[(size_t)jj * s->f_ldk + m] = H.sy[(size_t)jj * MC + (m == 0 ? 0 : 2 * m - 1)];
+                }
+            for (int m = 1; m <= L; m++)
+                for (int jj = 1; jj <= h - 1; jj++) {
+                    as[(size_t)(m - 1) * s->f_lds + (h - 1 - jj)] = H.an[(size_t)(2 * m) * Np + jj];
+                    ss[(size_t)jj * s->f_ldk + (m - 1)] = H.sy[(size_t)jj * MC + 2 * m];
+                }
+            if ((st = upload(&s->d_fAc, ac.data(), ac.size())) != SP_OK) return st;
+            if ((st = upload(&s->d_fAs, as.data(), as.size())) != SP_OK) return st;
+            if ((st = upload(&s->d_fSc, sc.data(), sc.size())) != SP_OK) return st;
+            if ((st = upload(&s->d_fSs, ss.data(), ss.size())) != SP_OK) return st;
+        }
     }
     if ((st = upload(&s->d_inv_r, H.inv_r.data(), Nr)) != SP_OK) return st;
     if ((st = upload(&s->d_sin_t, H.sin_t.data(), Nt)) != SP_OK) return st;
@@ -244,6 +265,7 @@ extern "C" sp_status sp_get_matrix(const sp_shell *s, int which, int n, int m, d
 #include "kernels_grad.cuh"
 #include "kernels_filter.cuh"
 #include "kernels_theta2.cuh"
+#include "kernels_fused.cuh"
 #include "kernels_wave.cuh"
 #include "kernels_ghg.cuh"
 
@@ -348,17 +370,23 @@ static size_t grad_smem_bytes(const sp_shell *s) {
     return ((size_t)2 * s->Nt8 * s->PU + (size_t)s->Nr8 * s->PU + 2 * s->Nt) * sizeof(double);
 }
 
+// Dynamic shared memory opt-in: the attribute belongs to the FUNCTION, process wide, not to a shell, so every instantiation is
+// opted in to the device maximum (227 KB) and a shell built later (smaller or larger) can never lower the cap of an earlier one.
+static const int SP_SMEM_MAX = 227 * 1024;
+
 sp_status sp_configure_kernels(sp_shell *s) {
     size_t sm = grad_smem_bytes(s);
     if (sm > 227 * 1024) return SP_ERR_UNSUPPORTED;       // (r,theta) plane pair must fit one SM's shared memory
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));
     {   // persistent (r,theta) kernel: two configurations, planes double-buffered (NBUF = 2) or not
         const int itiles = s->Nt8 / 8, ktiles = s->Nr8 / 8, KT = s->gradKT;
         const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
         s->grad_nwarps = (KT == 3) ? std::min(ntasks, 12) : std::min(ntasks, 6);
         cudaDeviceProp prop;
-        SP_CUDA(cudaGetDeviceProperties(&prop, 0));
+        int dev = 0;
+        SP_CUDA(cudaGetDevice(&dev));
+        SP_CUDA(cudaGetDeviceProperties(&prop, dev));
         s->num_sms = prop.multiProcessorCount;
         for (int nb = 1; nb <= 2; nb++) {
             s->grad_smem[nb - 1] = grad2_smem_bytes(s->Nt, s->Nt8, s->Nr8, s->PU, KT, nb, s->grad_nwarps);
@@ -366,11 +394,10 @@ sp_status sp_configure_kernels(sp_shell *s) {
         }
         if (s->grad_smem[0] > 227 * 1024) return SP_ERR_UNSUPPORTED;
 #define SP_GR_ATTR(KT_, SPL_, NB_)                                                                                      \
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<KT_, SPL_, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize,           \
-                                 (int)s->grad_smem[NB_ - 1]));                                                          \
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<KT_, SPL_, NB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));                                                          \
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta2<KT_, SPL_, NB_>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         SP_GR_ATTR(3, true, 1) SP_GR_ATTR(5, true, 1) SP_GR_ATTR(3, false, 1) SP_GR_ATTR(5, false, 1)
-        if (s->grad_smem[1] <= 227 * 1024) { SP_GR_ATTR(3, true, 2) SP_GR_ATTR(5, true, 2) SP_GR_ATTR(3, false, 2) SP_GR_ATTR(5, false, 2) }
+        SP_GR_ATTR(3, true, 2) SP_GR_ATTR(5, true, 2) SP_GR_ATTR(3, false, 2) SP_GR_ATTR(5, false, 2)
 #undef SP_GR_ATTR
         // resident CTAs per SM of the persistent grid, asked from the occupancy calculator for the variant that will run
         for (int nb = 1; nb <= 2; nb++) {
@@ -399,7 +426,7 @@ sp_status sp_configure_kernels(sp_shell *s) {
                 int occ = 0;
                 const int smb = (int)s->grad_smem[nb - 1];
 #define SP_G3P(KT_, NB_, PU_)                                                                                            \
-    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_, PU_>, cudaFuncAttributeMaxDynamicSharedMemorySize, smb));      \
+    SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_, PU_>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));      \
     SP_CUDA(cudaFuncSetAttribute(k_grad_rtheta3<KT_, NB_, PU_>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));   \
     SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grad_rtheta3<KT_, NB_, PU_>, thr, smb));
 #define SP_G3(KT_, NB_)                                                                      \
@@ -431,16 +458,16 @@ sp_status sp_configure_kernels(sp_shell *s) {
     PhiTiling tmax = {6, 4, 4 * 6 * 8};
     const int pg = (int)phi_smem_bytes(tmax);
 #define SP_PGA(MTV)                                                                                             \
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, false, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg)); \
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, false, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg));
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, false, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX)); \
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, false, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));
     SP_PGA(4) SP_PGA(5) SP_PGA(6)
 #undef SP_PGA
     {
         const size_t gfs = gradfold_smem_bytes(s->gf_Mpad, s->Np);
         s->gf_ok = s->gf_mg >= 1 && s->gf_mg <= 4 && gfs <= 227 * 1024;
         if (s->gf_ok) {
-            SP_CUDA(cudaFuncSetAttribute(k_phi_grad_fold<4, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gfs));
-            SP_CUDA(cudaFuncSetAttribute(k_phi_grad_fold<4, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gfs));
+            SP_CUDA(cudaFuncSetAttribute(k_phi_grad_fold<4, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));
+            SP_CUDA(cudaFuncSetAttribute(k_phi_grad_fold<4, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));
         }
     }
     {
@@ -449,8 +476,8 @@ sp_status sp_configure_kernels(sp_shell *s) {
         s->grad_split_ok = pgg <= 227 * 1024 && tg.mgroups <= 4;
         if (s->grad_split_ok) {
 #define SP_PGA(MTV)                                                                                                  \
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg)); \
-    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pgg));
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX)); \
+    SP_CUDA(cudaFuncSetAttribute(k_phi_gemm<MTV, true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));
             SP_PGA(4) SP_PGA(5) SP_PGA(6)
 #undef SP_PGA
         }
@@ -459,24 +486,25 @@ sp_status sp_configure_kernels(sp_shell *s) {
     if (theta2_smem_bytes(s->Nt8, true) <= 227 * 1024) {
         const int t1 = (int)theta2_smem_bytes(s->Nt8, false), t2 = (int)theta2_smem_bytes(s->Nt8, true);
 #define SP_TA(MTV, NTV)                                                                                           \
-    SP_CUDA(cudaFuncSetAttribute(k_theta2<MTV, NTV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t1));    \
-    SP_CUDA(cudaFuncSetAttribute(k_theta2<MTV, NTV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t2));
+    SP_CUDA(cudaFuncSetAttribute(k_theta2<MTV, NTV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));    \
+    SP_CUDA(cudaFuncSetAttribute(k_theta2<MTV, NTV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));
         SP_TA(1, 3) SP_TA(2, 3) SP_TA(3, 3) SP_TA(4, 3) SP_TA(1, 1) SP_TA(2, 1) SP_TA(3, 1) SP_TA(4, 1)
 #undef SP_TA
         if (s->d_G) {
             const int tf3 = (int)theta_fold_smem_bytes(s->h8, 3), tf1 = (int)theta_fold_smem_bytes(s->h8, 1);
 #define SP_TF(MTV)                                                                                                      \
-    if (tf3 <= 227 * 1024) SP_CUDA(cudaFuncSetAttribute(k_theta_fold<MTV, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tf3)); \
-    if (tf1 <= 227 * 1024) SP_CUDA(cudaFuncSetAttribute(k_theta_fold<MTV, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tf1));
+    SP_CUDA(cudaFuncSetAttribute(k_theta_fold<MTV, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX)); \
+    SP_CUDA(cudaFuncSetAttribute(k_theta_fold<MTV, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX));
             SP_TF(1) SP_TF(2) SP_TF(3) SP_TF(4)
 #undef SP_TF
         }
-        // measure, don't guess: time the candidate variants (warp tilings NT = 3 / 1, without and with the row-block split: codes 3, 1,
-        // 23, 21) on scratch data shaped like a GHG state (12 real + 18 complex components = 48 coefficient arrays), keep the winner
+        // Variant choice BY RULE (deterministic across processes, boxes and profilers): the table below is the outcome of timing
+        // runs on B200 (config 3, Ntheta = 48: NT = 3 unsplit; config 5, 64: NT = 1 split; config 4, 96: NT = 3
+        // split).  SP_THETA_NT forces a variant; SP_THETA_TUNE=1 re-runs the timing race on scratch data instead of the rule.
         const int cand[4] = {3, 1, 23, 21};
         bool ok[4];
         int nok = 0, only = 0;
-        const char *env = getenv("SP_THETA_NT");          // tuning override (profiling: a run under ncu distorts the timing below)
+        const char *env = getenv("SP_THETA_NT");
         const int forced = env ? atoi(env) : 0;
         for (int v = 0; v < 4; v++) {
             ok[v] = theta2_fits(s, cand[v]);
@@ -484,6 +512,15 @@ sp_status sp_configure_kernels(sp_shell *s) {
             if (ok[v] && forced == cand[v]) s->theta_NT = forced;
         }
         if (s->theta_NT == 0 && nok == 1) s->theta_NT = only;
+        const char *tune = getenv("SP_THETA_TUNE");
+        if (s->theta_NT == 0 && nok > 1 && !(tune && atoi(tune) == 1)) {
+            const int want = (s->Nt8 >= 88) ? 23 : (s->Nt8 >= 56) ? 21 : 3;
+            const int order[4] = {want, 3, 23, 21};
+            for (int q = 0; q < 4 && s->theta_NT == 0; q++)
+                for (int v = 0; v < 4; v++)
+                    if (ok[v] && cand[v] == order[q]) { s->theta_NT = cand[v]; break; }
+            if (s->theta_NT == 0) s->theta_NT = only;
+        }
         if (s->theta_NT == 0 && nok > 1) {
             const size_t dofsz = (size_t)s->MC4 * s->Nt * s->Nr;
             double *scr = nullptr;
@@ -720,8 +757,8 @@ static void tt_components(int tt, int dof0, std::vector<ThetaComp> &out) {
 }
 
 template <bool INV>
-static void launch_pointwise(const std::vector<int> &types, const std::vector<TensorArgs> &targs, const sp_shell *s, const double *src,
-                             double *dst, cudaStream_t st) {
+static void launch_pointwise(const std::vector<int> &types, const std::vector<TensorArgs> &targs, const std::vector<char> &sel,
+                             const sp_shell *s, const double *src, double *dst, cudaStream_t st) {
     const int T = 128;
     const unsigned nb = (unsigned)(((size_t)s->Nr * s->Nt * (s->Nt + 1) + T - 1) / T);
     std::vector<char> done(types.size(), 0);
@@ -729,13 +766,13 @@ static void launch_pointwise(const std::vector<int> &types, const std::vector<Te
     bool forked = false;
     int nlaunch = 0;
     for (size_t t0 = 0; t0 < types.size(); t0++) {
-        if (done[t0]) continue;
+        if (done[t0] || !sel[t0]) continue;
         // launches of different tensor groups are independent: every second one goes to the side stream
         if ((nlaunch++ & 1) && (forked || (forked = sp_fork(s, main_st)))) st = s->aux; else st = main_st;
         TensorArgsGroup tg;                      // this tensor and the following ones of the same index structure
         int n = 0;
         for (size_t t1 = t0; t1 < types.size() && n < SP_PW_GROUP; t1++)
-            if (!done[t1] && types[t1] == types[t0]) { tg.t[n++] = targs[t1]; done[t1] = 1; }
+            if (!done[t1] && sel[t1] && types[t1] == types[t0]) { tg.t[n++] = targs[t1]; done[t1] = 1; }
         const dim3 grid(nb, n);
 #define SP_PW(TTV)                                                                                                        \
     case TTV:                                                                                                             \
@@ -750,6 +787,182 @@ static void launch_pointwise(const std::vector<int> &types, const std::vector<Te
         g_sp_launches += 1;
     }
     if (forked) sp_join(s, main_st);
+}
+
+// ---- fused filter stages (kernels_fused.cuh) --------------------------------------------------------------------------------
+// Which tensors take the fused kernels.  Default (auto): tensors of up to 10 components (rank <= 2) whose data tiles leave three
+// CTAs per SM and whose launch group fills at least two CTAs per SM -- where the fused kernels are as fast as the five-stage path on
+// B200 and save its HBM round trips.  SP_FUSE = 0: never; 1: rank <= 2 whenever the tile fits; 2: every tensor
+// whose tile fits (rank 3: analysis side only).
+static int sp_fuse_mode() {
+    static const int v = [] { const char *e = getenv("SP_FUSE"); return e ? atoi(e) : -1; }();
+    return v;
+}
+static FusedParams fused_params(const sp_shell *s) {
+    FusedParams fp;
+    fp.Nr = s->Nr; fp.Nt = s->Nt; fp.L = s->L; fp.vec = s->Nr * s->Nt; fp.MC = s->MC;
+    fp.npts = (long)s->npts; fp.dofsz = (long)s->MC4 * fp.vec;
+    fp.sin_t = s->d_sin_t; fp.cos_t = s->d_cos_t; fp.sin_p = s->d_sin_p; fp.cos_p = s->d_cos_p;
+    fp.Ac = s->d_fAc; fp.As = s->d_fAs; fp.Mp = s->f_Mp; fp.ldc = s->f_ldc; fp.lds = s->f_lds;
+    fp.Sc = s->d_fSc; fp.Ss = s->d_fSs; fp.Jp = s->f_Jp; fp.ldk = s->f_ldk;
+    fp.WM = 1; fp.WN = 1; fp.ngroup = 1; fp.nbuf = 1; fp.zs = 1;
+    return fp;
+}
+// k_fan<TT, NC, MT, NTW, MAXT>: launch = true runs it, false only answers whether the tile fits
+// tile buffers of the fused kernels: 1 (default: one work item per CTA, grid = item count) or, with SP_FUSE_NBUF = 2, two: a persistent
+// grid whose CTAs stream the next item's tile in under the current item's products (measured slower on B200 at configs 2-5:
+// the second buffer costs a resident CTA per SM)
+static int fused_nbuf(size_t tile_bytes) {
+    static const int forced = [] { const char *e = getenv("SP_FUSE_NBUF"); return e ? atoi(e) : 0; }();
+    return (forced == 2 && 2 * tile_bytes <= (size_t)SP_SMEM_MAX) ? 2 : 1;
+}
+template <class K>
+static sp_status fused_grid(K kernel, int nthr, size_t smem, int nitems, int nbuf, const sp_shell *s, int &grid) {
+    grid = nitems;
+    if (nbuf < 2) return SP_OK;
+    int occ = 0;
+    SP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, nthr, smem));
+    if (occ < 1) return SP_ERR_CUDA;
+    grid = std::min(nitems, occ * s->num_sms);
+    return SP_OK;
+}
+template <int TT, int NC, int NTW, int MAXT>
+static sp_status fan_launch(const sp_shell *s, const TensorArgsGroup &tg, int n, const double *src, double *coef, cudaStream_t st, bool launch,
+                             size_t *tile_out, int *items_out) {
+    constexpr int nc = TTInfo<TT>::nc, ntiles = nc * NC / 8, WN = (ntiles + NTW - 1) / NTW;
+    static_assert(WN * 32 <= MAXT, "warp columns exceed the block size");
+    const int mtiles = s->f_Mp / 8;
+    const int MT = (nc > 10 || mtiles % 3 == 0 || mtiles >= 9) ? 3 : 2;
+    const int WM = std::max(1, std::min(std::min(4, MAXT / 32 / WN), (mtiles + MT - 1) / MT));
+    const size_t tile = fan_smem_bytes<NC>(nc, s->Np, 1);
+    if (tile > (size_t)SP_SMEM_MAX) return SP_ERR_UNSUPPORTED;
+    if (tile_out) *tile_out = tile;
+    if (items_out) *items_out = ((s->Nr * s->Nt + NC - 1) / NC) * n;
+    if (!launch) return SP_OK;
+    FusedParams fp = fused_params(s);
+    fp.WM = WM; fp.WN = WN; fp.ngroup = n; fp.nbuf = fused_nbuf(tile);
+    const size_t smem = fan_smem_bytes<NC>(nc, s->Np, fp.nbuf);
+    // further warps (up to SP_FAN_THREADS, default 128) only stage and project: the pointwise phase wants more threads than the products
+    static const int minthr = [] { const char *e = getenv("SP_FAN_THREADS"); return e ? atoi(e) : 128; }();
+    const int nthr = std::max(WM * WN * 32, std::min(MAXT, minthr));
+    const int nitems = ((fp.vec + NC - 1) / NC) * n;
+    int grid = 0;
+    sp_status e;
+    static bool attr3 = false, attr2 = false;
+    if (MT == 3) {
+        if (!attr3) { SP_CUDA(cudaFuncSetAttribute(k_fan<TT, NC, 3, NTW, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX)); attr3 = true; }
+        if ((e = fused_grid(k_fan<TT, NC, 3, NTW, MAXT>, nthr, smem, nitems, fp.nbuf, s, grid)) != SP_OK) return e;
+        k_fan<TT, NC, 3, NTW, MAXT><<<grid, nthr, smem, st>>>(tg, fp, src, coef);
+    } else {
+        if (!attr2) { SP_CUDA(cudaFuncSetAttribute(k_fan<TT, NC, 2, NTW, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX)); attr2 = true; }
+        if ((e = fused_grid(k_fan<TT, NC, 2, NTW, MAXT>, nthr, smem, nitems, fp.nbuf, s, grid)) != SP_OK) return e;
+        k_fan<TT, NC, 2, NTW, MAXT><<<grid, nthr, smem, st>>>(tg, fp, src, coef);
+    }
+    g_sp_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+static sp_status fan_dispatch(int tt, const sp_shell *s, const TensorArgsGroup &tg, int n, const double *src, double *coef, cudaStream_t st, bool launch,
+                               size_t *tile_out = nullptr, int *items_out = nullptr) {
+    // column tile and warp tiling per index structure: N = components x NC columns per CTA.  SP_FAN_NC4=1: 4-column tiles for the
+    // symmetric rank-2 types (experiments)
+    static const int nc4 = [] { const char *e = getenv("SP_FAN_NC4"); return e ? atoi(e) : 0; }();
+    // small states: narrower column tiles, so that the launch has at least ~2 CTAs per SM
+    const int vec = s->Nr * s->Nt;
+    const bool narrow = (long)((vec + 63) / 64) * std::max(n, 1) < 2L * s->num_sms;
+    const bool narrow16 = (long)((vec + 15) / 16) * std::max(n, 1) < 2L * s->num_sms;
+    switch (tt) {
+        case TT_SCALAR:
+            if (narrow) return fan_launch<TT_SCALAR, 16, 2, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+            return fan_launch<TT_SCALAR, 64, 4, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+        case TT_VEC3:
+            if (narrow16) return fan_launch<TT_VEC3, 8, 3, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+            return fan_launch<TT_VEC3, 16, 3, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+        case TT_VEC4:
+            if (narrow16) return fan_launch<TT_VEC4, 8, 4, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+            return fan_launch<TT_VEC4, 16, 4, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+        case TT_SYM3: return fan_launch<TT_SYM3, 8, 3, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+        case TT_SYM4:
+            if (nc4) return fan_launch<TT_SYM4, 4, 5, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+            return fan_launch<TT_SYM4, 8, 5, 512>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+        case TT_R3_3_3: return fan_launch<TT_R3_3_3, 4, 3, 256>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+        case TT_R3_3_4: return fan_launch<TT_R3_3_4, 4, 4, 256>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+        case TT_R3_4_3: return fan_launch<TT_R3_4_3, 4, 3, 256>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+        case TT_R3_4_4: return fan_launch<TT_R3_4_4, 4, 5, 256>(s, tg, n, src, coef, st, launch, tile_out, items_out);
+    }
+    return SP_ERR_UNSUPPORTED;
+}
+template <int TT, int CBW>
+static sp_status fsyn_launch(const sp_shell *s, const TensorArgsGroup &tg, int n, const double *coef, double *dst, cudaStream_t st, bool launch,
+                              size_t *tile_out, int *items_out) {
+    constexpr int nc = TTInfo<TT>::nc, NC = 8 * CBW;
+    // at most SP_FSYN_NW (default 4) warps per CTA: more CTAs along the longitudes share a column tile when there are more 8-row tiles
+    static const int nwmax = [] { const char *e = getenv("SP_FSYN_NW"); const int v = e ? atoi(e) : 4; return v >= 1 && v <= 8 ? v : 4; }();
+    const int jtiles = s->f_Jp / 8, zs = (jtiles + nwmax - 1) / nwmax, nw = (jtiles + zs - 1) / zs;
+    const size_t tile = fsyn_smem_bytes(nc, s->MC, NC, 1);
+    if (tile > (size_t)SP_SMEM_MAX) return SP_ERR_UNSUPPORTED;
+    if (tile_out) *tile_out = tile;
+    if (items_out) *items_out = ((s->Nr * s->Nt + NC - 1) / NC) * zs * n;
+    if (!launch) return SP_OK;
+    FusedParams fp = fused_params(s);
+    fp.ngroup = n; fp.zs = zs; fp.nbuf = fused_nbuf(tile);
+    const size_t smem = fsyn_smem_bytes(nc, s->MC, NC, fp.nbuf);
+    static bool attr = false;
+    if (!attr) { SP_CUDA(cudaFuncSetAttribute(k_fsyn<TT, CBW>, cudaFuncAttributeMaxDynamicSharedMemorySize, SP_SMEM_MAX)); attr = true; }
+    const int nitems = ((fp.vec + NC - 1) / NC) * zs * n;
+    int grid = 0;
+    sp_status e = fused_grid(k_fsyn<TT, CBW>, nw * 32, smem, nitems, fp.nbuf, s, grid);
+    if (e != SP_OK) return e;
+    k_fsyn<TT, CBW><<<grid, nw * 32, smem, st>>>(tg, fp, coef, dst);
+    g_sp_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+static sp_status fsyn_dispatch(int tt, const sp_shell *s, const TensorArgsGroup &tg, int n, const double *coef, double *dst, cudaStream_t st, bool launch,
+                                size_t *tile_out = nullptr, int *items_out = nullptr) {
+    const int vec = s->Nr * s->Nt;
+    const bool narrow = (long)((vec + 63) / 64) * std::max(n, 1) < 2L * s->num_sms;
+    const bool narrow16 = (long)((vec + 15) / 16) * std::max(n, 1) < 2L * s->num_sms;
+    switch (tt) {
+        case TT_SCALAR:
+            if (narrow) return fsyn_launch<TT_SCALAR, 2>(s, tg, n, coef, dst, st, launch, tile_out, items_out);
+            return fsyn_launch<TT_SCALAR, 8>(s, tg, n, coef, dst, st, launch, tile_out, items_out);
+        case TT_VEC3:
+            if (narrow16) return fsyn_launch<TT_VEC3, 1>(s, tg, n, coef, dst, st, launch, tile_out, items_out);
+            return fsyn_launch<TT_VEC3, 2>(s, tg, n, coef, dst, st, launch, tile_out, items_out);
+        case TT_VEC4:
+            if (narrow16) return fsyn_launch<TT_VEC4, 1>(s, tg, n, coef, dst, st, launch, tile_out, items_out);
+            return fsyn_launch<TT_VEC4, 2>(s, tg, n, coef, dst, st, launch, tile_out, items_out);
+        case TT_SYM3: return fsyn_launch<TT_SYM3, 1>(s, tg, n, coef, dst, st, launch, tile_out, items_out);
+        case TT_SYM4: return fsyn_launch<TT_SYM4, 1>(s, tg, n, coef, dst, st, launch, tile_out, items_out);
+    }
+    return SP_ERR_UNSUPPORTED;      // rank 3: the lane-local recombination would need > 255 registers; five-stage path
+}
+// joins the shell's side stream back into the caller's stream on every exit path (a fork left open would invalidate a CUDA
+// graph capture and hide the original error)
+struct AuxJoin {
+    const sp_shell *s; cudaStream_t st; bool open = false;
+    bool fork() { if (!open) open = sp_fork(s, st); return open; }
+    bool join() { if (!open) return true; open = false; return sp_join(s, st); }
+    ~AuxJoin() { if (open) sp_join(s, st); }
+};
+
+// run `fn(type, group, count, stream)` over the selected tensors, grouped by index structure (up to SP_PW_GROUP tensors per launch);
+// the launches of different groups are independent: every second one goes to the shell's side stream
+template <class Fn, class Aux>
+static sp_status for_groups(const std::vector<int> &types, const std::vector<TensorArgs> &targs, const std::vector<char> &sel,
+                            cudaStream_t st, Aux &aux, Fn fn) {
+    std::vector<char> done(types.size(), 0);
+    int nlaunch = 0;
+    for (size_t t0 = 0; t0 < types.size(); t0++) {
+        if (done[t0] || !sel[t0]) continue;
+        TensorArgsGroup tg;
+        int n = 0;
+        for (size_t t1 = t0; t1 < types.size() && n < SP_PW_GROUP; t1++)
+            if (!done[t1] && sel[t1] && types[t1] == types[t0]) { tg.t[n++] = targs[t1]; done[t1] = 1; }
+        const cudaStream_t sx = ((nlaunch++ & 1) && aux.fork()) ? aux.s->aux : st;
+        sp_status e = fn(types[t0], tg, n, sx);
+        if (e != SP_OK) return e;
+    }
+    return SP_OK;
 }
 
 extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double *out, int nfields, const sp_tensor_desc *tens,
@@ -790,28 +1003,70 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     const size_t need = (size_t)ndof * (npts + 2 * (size_t)s->MC4 * vec) * sizeof(double);
     if (!ws || wsb < need) return SP_ERR_INVALID_ARG;
     double *dofs = (double *)ws, *coef1 = dofs + (size_t)ndof * npts, *coef2 = coef1 + (size_t)ndof * s->MC4 * vec;
-    // ---- F1: dyad projection
-    sp_mark(s, st, 3);
-    launch_pointwise<false>(types, targs, s, u, dofs, st);
-    sp_mark(s, st, 4);
-    // ---- F2: phi analysis (eq. 33) on the folded rows: cosine block -> a_0..a_L, sine block -> b_1..b_L
-    auto phi = [&](const sp_shell::PhiMat &pm, const double *B, long sBb, double *C, long sCb, cudaStream_t sx) -> sp_status {
+    // ---- which tensors take the fused kernels (F1+F2 in k_fan, F4+F5 in k_fsyn): 16-byte aligned buffers, even strides, tile fits
+    std::vector<char> fanF(ntens, 0), synF(ntens, 0), fanU(ntens, 1), synU(ntens, 1);
+    const int fmode = sp_fuse_mode();
+    const bool fusable = fmode != 0 && s->d_fAc && !(vec & 1) && !(((uintptr_t)u | (uintptr_t)out | (uintptr_t)ws) & 15);
+    bool anyFanU = false, anySynU = false;
+    for (int t = 0; t < ntens; t++) {
+        if (fusable && (fmode > 1 || targs[t].ncomp <= 10)) {
+            TensorArgsGroup none;
+            int nsame = 0;                                   // tensors of this index structure: they share a launch
+            for (int q = 0; q < ntens; q++) nsame += types[q] == types[t];
+            nsame = std::min(nsame, SP_PW_GROUP);
+            size_t tf = 0, ts = 0;
+            int itf = 0, its = 0;
+            fanF[t] = fan_dispatch(types[t], s, none, nsame, nullptr, nullptr, st, false, &tf, &itf) == SP_OK;
+            synF[t] = fsyn_dispatch(types[t], s, none, nsame, nullptr, nullptr, st, false, &ts, &its) == SP_OK;
+            if (fmode < 0) {                                 // auto: both sides, three CTAs per SM, two CTAs per SM in flight
+                const size_t lim = (size_t)SP_SMEM_MAX / 3 - 1024;
+                const bool ok = fanF[t] && synF[t] && tf <= lim && ts <= lim && itf >= 2 * s->num_sms && its >= 2 * s->num_sms;
+                fanF[t] = synF[t] = ok;
+            }
+        }
+        fanU[t] = !fanF[t]; synU[t] = !synF[t];
+        anyFanU |= fanU[t] != 0; anySynU |= synU[t] != 0;
+    }
+    // contiguous dof ranges of the tensors that take the five-stage path (the phi products run per range)
+    auto ranges = [&](const std::vector<char> &sel) {
+        std::vector<std::pair<int, int>> r;
+        for (int t = 0; t < ntens; t++) {
+            if (!sel[t]) continue;
+            if (!r.empty() && r.back().first + r.back().second == targs[t].dof0) r.back().second += targs[t].ncomp;
+            else r.push_back({targs[t].dof0, targs[t].ncomp});
+        }
+        return r;
+    };
+    AuxJoin aux{s, st};
+    const long cst = (long)(s->MC4 * vec);
+    auto phi = [&](const sp_shell::PhiMat &pm, const double *B, long sBb, double *C, long sCb, int nb, cudaStream_t sx) -> sp_status {
         if (pm.M <= 0 || pm.K <= 0) return SP_OK;
         PhiTiling tl = {pm.MT, pm.mg, pm.Mpad};
-        sp_status e = launch_phi_gemm(pm.d, pm.K8, pm.M, tl, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, ndof, sx);
+        sp_status e = launch_phi_gemm(pm.d, pm.K8, pm.M, tl, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, nb, sx);
         if (e == SP_ERR_UNSUPPORTED)      // odd strides: generic global-memory kernel (same padded matrix)
-            e = launch_gemm_cols<false>(pm.d, pm.K8, pm.M, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, ndof, sx);
+            e = launch_gemm_cols<false>(pm.d, pm.K8, pm.M, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, nb, sx);
         g_sp_launches += 1;
         return e;
     };
-    const long cst = (long)(s->MC4 * vec);
-    // the cosine and the sine block are independent: the sine block runs on the side stream
-    bool fk = s->m_as.M > 0 && s->m_as.K > 0 && sp_fork(s, st);
-    sp_status e = phi(s->m_ac, dofs, (long)npts, coef1, cst, st);
+    sp_status e;
+    // ---- F1: dyad projection (five-stage tensors)
+    sp_mark(s, st, 3);
+    if (anyFanU) launch_pointwise<false>(types, targs, fanU, s, u, dofs, st);
+    sp_mark(s, st, 4);
+    // ---- F1 + F2 fused; F2: phi analysis (eq. 33) on the folded rows: cosine block -> a_0..a_L, sine block -> b_1..b_L
+    e = for_groups(types, targs, fanF, st, aux, [&](int tt, const TensorArgsGroup &tg, int n, cudaStream_t sx) { return fan_dispatch(tt, s, tg, n, u, coef1, sx, true); });
     if (e != SP_OK) return e;
-    e = phi(s->m_as, dofs + (size_t)(Nt + 1) * vec, (long)npts, coef1 + (size_t)(s->L + 1) * vec, cst, fk ? s->aux : st);
-    if (e != SP_OK) return e;
-    if (fk && !sp_join(s, st)) return SP_ERR_CUDA;
+    if (anyFanU) {
+        // the cosine and the sine block are independent: the sine block runs on the side stream
+        const bool fk = s->m_as.M > 0 && s->m_as.K > 0 && aux.fork();
+        for (const auto &r : ranges(fanU)) {
+            const double *B = dofs + (size_t)r.first * npts;
+            double *C = coef1 + (size_t)r.first * cst;
+            if ((e = phi(s->m_ac, B, (long)npts, C, cst, r.second, st)) != SP_OK) return e;
+            if ((e = phi(s->m_as, B + (size_t)(Nt + 1) * vec, (long)npts, C + (size_t)(s->L + 1) * vec, cst, r.second, fk ? s->aux : st)) != SP_OK) return e;
+        }
+    }
+    if (!aux.join()) return SP_ERR_CUDA;      // fused launches on the side stream and the sine blocks are back before the theta step
     sp_mark(s, st, 5);
     // ---- F3: per-(n,m) theta matrices (eq. 62)
     {
@@ -836,19 +1091,25 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
     }
     sp_mark(s, st, 6);
-    // ---- F4: phi synthesis (eq. 31) into the folded rows: e_j (cosine block), o_j (sine block)
-    fk = s->m_ss.M > 0 && s->m_ss.K > 0 && sp_fork(s, st);
-    e = phi(s->m_sc, coef2, cst, dofs, (long)npts, st);
+    // ---- F4 + F5 fused; F4: phi synthesis (eq. 31) into the folded rows: e_j (cosine block), o_j (sine block)
+    e = for_groups(types, targs, synF, st, aux, [&](int tt, const TensorArgsGroup &tg, int n, cudaStream_t sx) { return fsyn_dispatch(tt, s, tg, n, coef2, out, sx, true); });
     if (e != SP_OK) return e;
-    e = phi(s->m_ss, coef2 + (size_t)(s->L + 1) * vec, cst, dofs + (size_t)(Nt + 1) * vec, (long)npts, fk ? s->aux : st);
-    if (e != SP_OK) return e;
-    if (fk && !sp_join(s, st)) return SP_ERR_CUDA;
-    if (s->m_ss.K <= 0 && Nt > 1)      // L = 0: no sine modes survive, the odd rows o_j are zero
-        SP_CUDA(cudaMemset2DAsync(dofs + (size_t)(Nt + 1) * vec, npts * sizeof(double), 0, (size_t)(Nt - 1) * vec * sizeof(double),
-                                  (size_t)ndof, st));
+    if (anySynU) {
+        const bool fk = s->m_ss.M > 0 && s->m_ss.K > 0 && aux.fork();
+        for (const auto &r : ranges(synU)) {
+            const double *C = coef2 + (size_t)r.first * cst;
+            double *B = dofs + (size_t)r.first * npts;
+            if ((e = phi(s->m_sc, C, cst, B, (long)npts, r.second, st)) != SP_OK) return e;
+            if ((e = phi(s->m_ss, C + (size_t)(s->L + 1) * vec, cst, B + (size_t)(Nt + 1) * vec, (long)npts, r.second, fk ? s->aux : st)) != SP_OK) return e;
+            if (s->m_ss.K <= 0 && Nt > 1)      // L = 0: no sine modes survive, the odd rows o_j are zero
+                SP_CUDA(cudaMemset2DAsync(B + (size_t)(Nt + 1) * vec, npts * sizeof(double), 0, (size_t)(Nt - 1) * vec * sizeof(double),
+                                          (size_t)r.second, st));
+        }
+    }
+    if (!aux.join()) return SP_ERR_CUDA;
     sp_mark(s, st, 7);
-    // ---- F5: recombination
-    launch_pointwise<true>(types, targs, s, dofs, out, st);
+    // ---- F5: recombination (five-stage tensors)
+    if (anySynU) launch_pointwise<true>(types, targs, synU, s, dofs, out, st);
     sp_mark(s, st, 8);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
@@ -904,6 +1165,17 @@ extern "C" sp_status sp_ghg_init(const sp_shell *s, double *u, double *H, void *
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
 
+extern "C" sp_status sp_wave_dt(const sp_shell *s, double lambda, double *dt) {
+    if (!s || !dt || !(lambda > 0)) return SP_ERR_INVALID_ARG;
+    const double PI = 3.14159265358979323846;
+    const double mid = 0.5 * (s->rout + s->rin), half = 0.5 * (s->rout - s->rin);
+    const double r0 = mid - half, r1 = mid - half * cos(PI / (s->Nr - 1));                 // eq. 2
+    const double th0 = PI * 0.5 / s->Nt;                                                   // eq. 3
+    const double dphi = 2.0 * r0 * sin(th0) * sin(PI / s->Np);
+    *dt = lambda * std::min(r1 - r0, dphi);                                                // eq. 63
+    return SP_OK;
+}
+
 extern "C" sp_status sp_axpby(double a, const double *x, double b, double *y, size_t n, void *stream) {
     if (!x || !y) return SP_ERR_INVALID_ARG;
     if (n == 0) return SP_OK;
@@ -930,7 +1202,9 @@ extern "C" sp_status sp_rk4_stage(const double *u, const double *k, const double
 extern "C" sp_status sp_probe_fp64_peak(int mode, double *tflops) {
     if (!tflops || mode < 0 || mode > 1) return SP_ERR_INVALID_ARG;
     cudaDeviceProp prop;
-    SP_CUDA(cudaGetDeviceProperties(&prop, 0));
+    int dev = 0;
+    SP_CUDA(cudaGetDevice(&dev));
+    SP_CUDA(cudaGetDeviceProperties(&prop, dev));
     const int grid = prop.multiProcessorCount * 2, thr = 512, iters = 20000;
     double *buf = nullptr;
     SP_CUDA(cudaMalloc((void **)&buf, sizeof(double) * grid * thr));

@@ -4,15 +4,12 @@ Host-side sequencing only: every arithmetic step is a kernel behind the C ABI
 (sp_rhs_first_order_wave, sp_axpby, sp_tensor_filter).  Filter placement (reading W5):
 the initial data, every stage state before its RHS, and the final combination -- 4 filters per step.
 """
-import math
 
 
 def wave_dt(Nr, Nt, Np, r_in, r_out, lam=4.0):
-    """dt = lambda * min(dx), eq. 63 (reading W4)."""
-    r0 = 0.5 * (r_out + r_in) - 0.5 * (r_out - r_in)
-    r1 = 0.5 * (r_out + r_in) - 0.5 * (r_out - r_in) * math.cos(math.pi / (Nr - 1))
-    th0 = math.pi * 0.5 / Nt
-    return lam * min(r1 - r0, 2.0 * r0 * math.sin(th0) * math.sin(math.pi / Np))
+    """dt = lambda * min(dx), eq. 63 (reading W4): computed behind the C ABI (sp_wave_dt); this is marshalling only."""
+    from .binding import Shell
+    return Shell(Nr, Nt, Np, r_in, r_out, 0, build=False).wave_dt(lam)
 
 
 class WaveRK4:

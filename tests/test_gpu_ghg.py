@@ -122,7 +122,7 @@ def test_ghg_rk4_parity_with_oracle():
     rk = GhgRK4(sh, torch.from_numpy(H).cuda(), torch.from_numpy(dH).cuda())
     got = rk.evolve(torch.from_numpy(u0).cuda(), dt, 3).cpu().numpy()
     want = _oracle_rk4(u0, H, dH, Nr, Nt, Np, L, dt, 3)
-    assert _rel(got, want) < 3e-12
+    assert _rel(got, want) < TOL
     got_g = rk.evolve(torch.from_numpy(u0).cuda(), dt, 3, graph=True).cpu().numpy()
     assert np.array_equal(got_g, got)
 

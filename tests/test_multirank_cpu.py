@@ -43,3 +43,19 @@ def test_single_rank_passthrough():
     assert bench.aggregate_over_ranks(3.0, 7.0, None) == (3.0, 7.0)
     fl = bench.flops_per_unit({"Nr": 33, "Nt": 48, "Np": 96, "L": 43})
     assert sum(fl.values()) == (2 * 33 + 4 * 48 + 2 * 96 + 13) + 5 * (2 * 43 + 1)
+
+
+def test_gpus_2_without_torchrun_starts_two_ranks():
+    """`python bench.py --gpus 2` launched plainly (no torchrun, WORLD_SIZE unset) must start the two ranks itself.  Driven end
+    to end on the CPU through the reference arm: both ranks rendezvous over gloo, rank 0 alone runs the oracle and prints the
+    one JSON line with n_gpus = 2."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--config", "1",
+                        "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=600, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.strip().splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
