@@ -417,6 +417,26 @@ class GpuWorkload:
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) / steps
 
+    def latency_floor_ms(self, nlaunch, reps=200):
+        """Launch/latency floor of a step: a CUDA graph of `nlaunch` DEPENDENT near-empty kernels (one 8-byte fill each) replayed
+        back to back -- what a step of that many launches costs on this device when every kernel has nothing to do."""
+        torch = self.torch
+        x = torch.zeros(1, dtype=torch.float64, device="cuda")
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(nlaunch):
+                x.add_(1.0)
+        g.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
     def time_call_graph(self, which, steps, warmup=1):
         """The same call alone, replayed from a CUDA graph holding one call per input copy (the headline's launch mode)."""
         torch = self.torch
@@ -733,20 +753,21 @@ def roofline_for(cfg, stages_ms, units, peak_tf, hbm_gbs, hbm_src):
         table[k] = {"ms": ms, "tflops": fl[k] * units / (ms * 1e-3) * 1e-12}
     dom = max(table, key=lambda k: table[k]["ms"])
     ach = table[dom]["tflops"]
-    traffic, executed = None, {}
+    traffic, executed, tsrc = None, {}, None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
         try:
             tj = json.load(open(tp))
             traffic = tj.get(f"config{cfg['id']}", {}).get(dom)
             executed = tj.get(f"config{cfg['id']}_executed_flops", {})
+            tsrc = tj.get("source")
         except Exception:
-            traffic, executed = None, {}
+            traffic, executed, tsrc = None, {}, None
     for k in table:                      # executed (ncu instruction counts, profiles/) next to the algorithmic count
         if k in executed:
             table[k]["executed_tflops"] = executed[k] / (table[k]["ms"] * 1e-3) * 1e-12
     roof = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-            "traffic": traffic,
+            "traffic": traffic, "traffic_source": tsrc,
             "achieved_executed": table[dom].get("executed_tflops"),
             "frac_executed": (table[dom]["executed_tflops"] / peak_tf) if "executed_tflops" in table[dom] else None,
             "executed_flops_per_step": sum(executed.values()) if executed else None,
@@ -878,6 +899,15 @@ def run_ours(args):
                                       "stages_ms": {k: v["ms"] for k, v in t2.items()}}
             others[f"config{cid}"]["calls"] = w2.calls_report(max(10, k2 // 4), peak_tf)
             if cid in (2, 5):  # these states fit L2: the figure above rotates inputs (HBM-cold); this one re-reads one copy
+                from paper_1104_3408_b200 import launch_count
+                l0 = launch_count()
+                w2.step()
+                nl = launch_count() - l0
+                torch.cuda.synchronize()
+                others[f"config{cid}"]["launches_per_step"] = nl
+                # the gradient chain and the filter chain run side by side: the floor is the longer chain (about half the launches)
+                others[f"config{cid}"]["latency_floor_ms"] = {"all_launches_in_one_chain": w2.latency_floor_ms(nl),
+                                                              "half_of_them_per_chain": w2.latency_floor_ms((nl + 1) // 2)}
                 w2.nsets = 1
                 others[f"config{cid}"]["ms_per_step_l2_warm"] = timed(w2, k2, 3) / k2
             if cid == 5:      # the configuration's own workload: 200 RK4 steps with the Yn filter after every substep

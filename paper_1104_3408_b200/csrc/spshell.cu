@@ -590,12 +590,24 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     p.u = u; p.dphi = nullptr; p.du = du; p.nf = nf; p.nitems = Nt * nf;
     const dim3 grid(Nt, nf);
     PhiTiling tl = {s->fd3_MT, s->fd3_mg, s->fd3_Mpad};
-    g_sp_launches += 2;
     sp_mark(s, st, 0);
     // ---- fast path: (r,theta)-plane kernel first (W -> du[x], d_z -> du[z]), then the d/dphi GEMM whose epilogue
     //      applies the chain rule (eq. 6).  Needs Ntheta % 4 == 0, even strides and 16-byte aligned buffers.
     const bool aligned = !(((uintptr_t)u | (uintptr_t)du) & 15) && !((plane | (long)s->npts) & 1);
     if (Nt % 4 == 0 && s->grad_split_ok && aligned) {
+      // SP_GRAD_CHUNK = c > 0: run the two kernels over chunks of c fields, so that a chunk's input and its intermediate W (written
+      // by the plane kernel into the d_x slot, re-read by the d/dphi epilogue) are still in the 126 MB L2 when the second kernel
+      // runs.  Off by default: measured slower on B200 -- the persistent plane kernel loses its pipelining
+      // on short item lists.
+      static const int chunk_env = [] { const char *e = getenv("SP_GRAD_CHUNK"); return e ? atoi(e) : 0; }();
+      const int nf_all = nf, chunk = (chunk_env > 0 && chunk_env < nf) ? chunk_env : nf;
+      const double *u_all = u;
+      double *du_all = du;
+      for (int f0 = 0; f0 < nf_all; f0 += chunk) {
+        const int nf = std::min(chunk, nf_all - f0);
+        const double *u = u_all + (size_t)f0 * s->npts;
+        double *du = du_all + (size_t)f0 * s->npts;
+        p.u = u; p.du = du; p.nf = nf_all; p.nitems = Nt * nf;
         const int KT = s->gradKT;
         const int ntasks = 2 * ((itiles + 1) / 2) * ((ktiles + KT - 1) / KT);
         if (s->grad3_ctas[0] > 0) {      // folded theta derivative (k_grad_rtheta3)
@@ -636,7 +648,7 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
         }
         if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         sp_mark(s, st, 1);
-        PhiGradEpi ge = {du + (size_t)nf * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
+        PhiGradEpi ge = {du + (size_t)nf_all * s->npts, (long)s->npts, s->d_inv_r, s->d_inv_sin_t, s->d_sin_p, s->d_cos_p, Nr};
         // the fold halves the DMMAs but doubles the rows each warp finishes; measured: it wins from Nphi = 128 upwards
         if (s->gf_ok && Np >= sp_dphi_fold_min()) {      // reflection-folded d/dphi with the chain rule in the epilogue
             // 32-column tiles for this kernel at every size (config 4: 0.97 -> 0.88 ms; small states use them anyway)
@@ -664,12 +676,15 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
                                           st, &ge);
             if (e != SP_OK) return e;
         }
+        g_sp_launches += 2;
+      }
         sp_mark(s, st, 2);
         s->grad_swapped = true;
         return SP_OK;
     }
     // ---- general path: d/dphi into the workspace, then the plane kernel finishes all three components
     s->grad_swapped = false;
+    g_sp_launches += 2;
     double *dphi = (double *)ws;
     p.dphi = dphi;
     sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
