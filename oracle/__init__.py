@@ -254,3 +254,73 @@ def ghg_lapse_shift(u, Nr, Nt, Np):
     out = np.zeros((10, Np, Nt, Nr))
     lib().orc_ghg_lapse_shift(C.c_int(Nr), C.c_int(Nt), C.c_int(Np), u.ctypes, out.ctypes)
     return out
+
+
+# ---- nested shells (DESIGN.md section 11 readings N1-N4) ----
+# The paper names domain decomposition into nested shells as future work and specifies nothing.  Reading: shells
+# [R_a, R_a+1] share their interface spheres and the angular grid (the interface points coincide, no interpolation); each shell
+# is evolved as in the single-shell case and the shells are coupled through the characteristic fields of (A.13)-(A.16)
+# on the shared sphere: with n = r^, U^+ = Pi + n.Phi moves outward and U^- = Pi - n.Phi inward; each side
+# keeps the RHS of the field that LEAVES it and takes the RHS of the field that ENTERS it from its neighbour, i.e. (A.16) with
+# the zeroed incoming part replaced by the neighbour's; the zero-speed fields (psi, tangential Phi) keep their own RHS.
+def wave_rhs_raw(u, Nr, Nt, Np, rmin, rmax):
+    """(-Pi, -d_i Phi_i, -d_x Pi, -d_y Pi, -d_z Pi) on one shell from the oracle gradient, no boundary treatment."""
+    u, nf = _state(u, Nr, Nt, Np)
+    assert nf == 5
+    u = u.reshape(5, Np, Nt, Nr)
+    g = gradient(u[1:], Nr, Nt, Np, rmin, rmax)                  # [3, 4 (Pi, Phi_x, Phi_y, Phi_z), Np, Nt, Nr]
+    return np.stack([-u[1], -(g[0, 1] + g[1, 2] + g[2, 3]), -g[0, 0], -g[1, 0], -g[2, 0]])
+
+
+def _unit_normal(Nt, Np):
+    th = np.pi * (np.arange(Nt) + 0.5) / Nt
+    ph = 2.0 * np.pi * np.arange(Np) / Np
+    PH, TH = np.meshgrid(ph, th, indexing="ij")
+    return np.stack([np.sin(TH) * np.cos(PH), np.sin(TH) * np.sin(PH), np.cos(TH)])      # [3, Np, Nt]
+
+
+def nested_wave_rhs(us, shells):
+    """us[a]: state [5, Np, Nt, Nr_a] of shell a; shells[a] = dict(Nr, Nt, Np, rmin, rmax), shells[a]['rmax'] == shells[a+1]['rmin'].
+    Freezing condition (A.16) on the innermost and outermost sphere, characteristic exchange on every interface."""
+    n = _unit_normal(shells[0]["Nt"], shells[0]["Np"])
+    raw = [wave_rhs_raw(u, s["Nr"], s["Nt"], s["Np"], s["rmin"], s["rmax"]) for u, s in zip(us, shells)]
+    out = [r.copy() for r in raw]
+
+    def put(d, k, dPi, ndPhi, own):
+        """row k of d: Pi-RHS dPi, normal part of the Phi-RHS ndPhi, tangential part and psi from `own`"""
+        tang = own[2:5, ..., k] - n * np.sum(n * own[2:5, ..., k], axis=0)
+        d[1, ..., k] = dPi
+        d[2:5, ..., k] = tang + n * ndPhi
+
+    for a in range(len(shells) - 1):
+        assert shells[a]["rmax"] == shells[a + 1]["rmin"] and shells[a]["Nt"] == shells[a + 1]["Nt"]
+        A, B = raw[a], raw[a + 1]
+        Up = A[1, ..., -1] + np.sum(n * A[2:5, ..., -1], axis=0)     # leaves shell a outward, enters shell a+1
+        Um = B[1, ..., 0] - np.sum(n * B[2:5, ..., 0], axis=0)       # leaves shell a+1 inward, enters shell a
+        put(out[a], -1, 0.5 * (Up + Um), 0.5 * (Up - Um), A)
+        put(out[a + 1], 0, 0.5 * (Up + Um), 0.5 * (Up - Um), B)
+    first, last = raw[0], raw[-1]
+    Um = first[1, ..., 0] - np.sum(n * first[2:5, ..., 0], axis=0)   # inner physical boundary: the outward-moving U^+ enters: frozen
+    put(out[0], 0, 0.5 * Um, -0.5 * Um, first)
+    Up = last[1, ..., -1] + np.sum(n * last[2:5, ..., -1], axis=0)   # outer physical boundary: the inward-moving U^- enters: frozen
+    put(out[-1], -1, 0.5 * Up, 0.5 * Up, last)
+    return out
+
+
+def nested_wave_dt(shells, lam=4.0):
+    return min(wave_dt(s["Nr"], s["Nt"], s["Np"], s["rmin"], s["rmax"], lam) for s in shells)
+
+
+def nested_wave_rk4(us, shells, L, tensors, dt, nsteps):
+    """Classical RK4 of the coupled shells, Yn filter per shell at the places of wave_rk4 (reading W5)."""
+    F = lambda vs: [tensor_filter(v, s["Nr"], s["Nt"], s["Np"], L, tensors) for v, s in zip(vs, shells)]
+    R = lambda vs: nested_wave_rhs(vs, shells)
+    ax = lambda vs, c, ks: [v + c * k for v, k in zip(vs, ks)]
+    us = F([np.array(u, dtype=np.float64) for u in us])
+    for _ in range(nsteps):
+        k1 = R(us)
+        k2 = R(F(ax(us, 0.5 * dt, k1)))
+        k3 = R(F(ax(us, 0.5 * dt, k2)))
+        k4 = R(F(ax(us, dt, k3)))
+        us = F([u + dt / 6.0 * (a + 2.0 * b + 2.0 * c + d) for u, a, b, c, d in zip(us, k1, k2, k3, k4)])
+    return us
