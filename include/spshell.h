@@ -130,6 +130,22 @@ sp_status sp_rhs_ghg(const sp_shell *shell, const double *u_dev, const double *H
  * 20..49); fills k_ab = (beta^i/alpha) d_iab (A.6) into fields 10..19 and H_a = -Gamma_a (A.18) into H (4 fields). */
 sp_status sp_ghg_init(const sp_shell *shell, double *u_dev, double *H_dev, void *cuda_stream);
 
+/* Nested shells (PAPER.md:39, 616 name them as future work and specify nothing: DESIGN.md section 11).
+ * sp_rhs_wave_shell is sp_rhs_first_order_wave with the boundary treatment chosen per boundary sphere: bc_inner / bc_outer = 1
+ * applies the freezing condition (A.16) on k = 0 / k = Nr-1 (a physical boundary), 0 leaves the raw right-hand side there (an
+ * interface with a neighbouring shell, to be coupled by sp_wave_interface).  Same arguments, workspace and errors otherwise. */
+sp_status sp_rhs_wave_shell(const sp_shell *shell, const double *u_dev, double *dudt_dev, int bc_inner, int bc_outer,
+                            void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Characteristic coupling of two shells on their shared sphere r = inner.r_out = outer.r_in ((A.13)-(A.16) with
+ * the zeroed incoming part replaced by the neighbour's): with n = r^, U+ = Pi + n.Phi (moving outward) is taken from the inner
+ * shell's raw RHS row k = Nr_inner-1, U- = Pi - n.Phi (moving inward) from the outer shell's raw RHS row k = 0; BOTH rows get
+ * d_t Pi = (U+ + U-)/2 and the normal part n.d_t Phi = (U+ - U-)/2; the tangential part of d_t Phi and d_t psi stay each shell's
+ * own.  dudt_inner_dev / dudt_outer_dev: [5] state-shaped RHS arrays of the two shells (raw on the shared sphere), updated in
+ * place.  The shells must share Ntheta and Nphi and the radius (SP_ERR_INVALID_ARG otherwise).  Asynchronous, allocates nothing. */
+sp_status sp_wave_interface(const sp_shell *inner, double *dudt_inner_dev, const sp_shell *outer, double *dudt_outer_dev,
+                            void *cuda_stream);
+
 /* Time step of the method of lines, eq. (63) (reading W4): dt = lambda * min(dx) with min(dx) the
  * smaller of the first radial spacing r_1 - r_0 and the azimuthal spacing 2 r_0 sin(theta_0) sin(pi / Nphi) on the innermost
  * sphere next to the pole.  Host arithmetic on the shell's grid parameters; no device, no build needed.  lambda <= 0 is

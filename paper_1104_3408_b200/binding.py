@@ -8,7 +8,7 @@ _lib = None
 # every symbol include/spshell.h declares
 EXPORTED_SYMBOLS = [
     "sp_shell_create", "sp_shell_destroy", "sp_build_matrices", "sp_workspace_bytes", "sp_cartesian_gradient",
-    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_wave_dt", "sp_axpby", "sp_rk4_stage", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
+    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_rhs_wave_shell", "sp_wave_interface", "sp_wave_dt", "sp_axpby", "sp_rk4_stage", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
     "sp_status_string", "sp_profile_enable", "sp_profile_read", "sp_launch_count",
 ]
 
@@ -44,6 +44,8 @@ def lib():
         L.sp_tensor_filter.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(_TensorDesc), C.c_int,
                                        C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rhs_first_order_wave.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sp_rhs_wave_shell.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sp_wave_interface.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.sp_wave_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.sp_axpby.argtypes = [C.c_double, C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rk4_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_size_t,
@@ -217,6 +219,27 @@ class Shell:
         _check(lib().sp_rhs_first_order_wave(self._h, u.data_ptr(), out.data_ptr(), ws.data_ptr(), ws.numel() * 8,
                                              _stream_ptr(stream)), "sp_rhs_first_order_wave")
         return out
+
+    def rhs_wave_shell(self, u, bc_inner=True, bc_outer=True, out=None, workspace=None, stream=None):
+        """sp_rhs_wave_shell: the scalar-wave RHS with the freezing condition only on the physical boundary spheres."""
+        import torch
+        u = _dev_f64(u, "u")
+        if u.numel() != 5 * self.npts:
+            raise SpError("u must hold the 5 fields psi, Pi, Phi_x, Phi_y, Phi_z")
+        if out is None:
+            out = torch.empty_like(u)
+        need = self.workspace_bytes(5)[2]
+        ws = self._workspace(need, u.device) if workspace is None else _dev_f64(workspace, "workspace")
+        _check(lib().sp_rhs_wave_shell(self._h, u.data_ptr(), out.data_ptr(), 1 if bc_inner else 0, 1 if bc_outer else 0,
+                                       ws.data_ptr(), ws.numel() * 8, _stream_ptr(stream)), "sp_rhs_wave_shell")
+        return out
+
+    @staticmethod
+    def wave_interface(inner, dudt_inner, outer, dudt_outer, stream=None):
+        """sp_wave_interface: characteristic coupling of two shells on their shared sphere (both RHS arrays updated in place)."""
+        _dev_f64(dudt_inner, "dudt_inner"); _dev_f64(dudt_outer, "dudt_outer")
+        _check(lib().sp_wave_interface(inner._h, dudt_inner.data_ptr(), outer._h, dudt_outer.data_ptr(), _stream_ptr(stream)),
+               "sp_wave_interface")
 
     def wave_dt(self, lam=4.0):
         """dt = lambda * min(dx), eq. 63 (sp_wave_dt)."""

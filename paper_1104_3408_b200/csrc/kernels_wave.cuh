@@ -11,7 +11,7 @@
 __global__ void __launch_bounds__(256)
 k_wave_rhs(int Nr, int Nt, size_t npts, const double *__restrict__ sin_t, const double *__restrict__ cos_t,
            const double *__restrict__ sin_p, const double *__restrict__ cos_p, const double *__restrict__ u,
-           const double *__restrict__ dg, double *__restrict__ dudt) {
+           const double *__restrict__ dg, double *__restrict__ dudt, int bcmask) {
     const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npts) return;
     const int k = (int)(p % Nr), i = (int)((p / Nr) % Nt), j = (int)(p / ((size_t)Nr * Nt));
@@ -19,7 +19,7 @@ k_wave_rhs(int Nr, int Nt, size_t npts, const double *__restrict__ sin_t, const 
     double dpsi = -u[npts + p];
     double dPi = -(D(0, 1) + D(1, 2) + D(2, 3));
     double dPh[3] = {-D(0, 0), -D(1, 0), -D(2, 0)};
-    if (k == 0 || k == Nr - 1) {
+    if ((k == 0 && (bcmask & 1)) || (k == Nr - 1 && (bcmask & 2))) {      // bcmask: bit 0 inner, bit 1 outer sphere is a physical boundary
         const double sg = (k == 0) ? -1.0 : 1.0;
         const double s[3] = {sg * sin_t[i] * cos_p[j], sg * sin_t[i] * sin_p[j], sg * cos_t[i]};
         const double sd = s[0] * dPh[0] + s[1] * dPh[1] + s[2] * dPh[2];
@@ -33,6 +33,32 @@ k_wave_rhs(int Nr, int Nt, size_t npts, const double *__restrict__ sin_t, const 
     dudt[2 * npts + p] = dPh[0];
     dudt[3 * npts + p] = dPh[1];
     dudt[4 * npts + p] = dPh[2];
+}
+
+// Characteristic coupling of two shells on their shared sphere (spshell.h: sp_wave_interface).  One thread per (i, j); a = the inner
+// shell's RHS row k = Nra-1, b = the outer shell's row k = 0, both raw on entry.
+__global__ void __launch_bounds__(128)
+k_wave_interface(int Nt, int Np, int Nra, int Nrb, const double *__restrict__ sin_t, const double *__restrict__ cos_t,
+                 const double *__restrict__ sin_p, const double *__restrict__ cos_p, double *da, double *db) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= Nt * Np) return;
+    const int i = q % Nt, j = q / Nt;
+    const size_t na = (size_t)Nra * Nt * Np, nb = (size_t)Nrb * Nt * Np;
+    const size_t pa = (size_t)q * Nra + (Nra - 1), pb = (size_t)q * Nrb;
+    const double n[3] = {sin_t[i] * cos_p[j], sin_t[i] * sin_p[j], cos_t[i]};
+    const double aPi = da[na + pa], bPi = db[nb + pb];
+    double aPh[3], bPh[3];
+#pragma unroll
+    for (int c = 0; c < 3; c++) { aPh[c] = da[(2 + c) * na + pa]; bPh[c] = db[(2 + c) * nb + pb]; }
+    const double nA = n[0] * aPh[0] + n[1] * aPh[1] + n[2] * aPh[2], nB = n[0] * bPh[0] + n[1] * bPh[1] + n[2] * bPh[2];
+    const double Up = aPi + nA, Um = bPi - nB;          // leaves the inner shell outward / leaves the outer shell inward
+    const double dPi = 0.5 * (Up + Um), nd = 0.5 * (Up - Um);
+    da[na + pa] = dPi; db[nb + pb] = dPi;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        da[(2 + c) * na + pa] = aPh[c] + n[c] * (nd - nA);
+        db[(2 + c) * nb + pb] = bPh[c] + n[c] * (nd - nB);
+    }
 }
 
 __global__ void __launch_bounds__(256) k_axpby(double a, const double *__restrict__ x, double b, double *__restrict__ y, size_t n) {

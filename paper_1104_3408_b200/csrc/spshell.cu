@@ -1129,7 +1129,8 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
 
-extern "C" sp_status sp_rhs_first_order_wave(const sp_shell *s, const double *u, double *dudt, void *ws, size_t wsb, void *stream) {
+extern "C" sp_status sp_rhs_wave_shell(const sp_shell *s, const double *u, double *dudt, int bc_inner, int bc_outer, void *ws, size_t wsb,
+                                       void *stream) {
     if (!s || !u || !dudt) return SP_ERR_INVALID_ARG;
     if (!s->built) return SP_ERR_NOT_BUILT;
     const size_t npts = s->npts;
@@ -1140,7 +1141,22 @@ extern "C" sp_status sp_rhs_first_order_wave(const sp_shell *s, const double *u,
     const int T = 256;
     g_sp_launches += 1;
     k_wave_rhs<<<(unsigned)((npts + T - 1) / T), T, 0, (cudaStream_t)stream>>>(s->Nr, s->Nt, npts, s->d_sin_t, s->d_cos_t, s->d_sin_p,
-                                                                              s->d_cos_p, u, dg, dudt);
+                                                                              s->d_cos_p, u, dg, dudt, (bc_inner ? 1 : 0) | (bc_outer ? 2 : 0));
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
+}
+
+extern "C" sp_status sp_rhs_first_order_wave(const sp_shell *s, const double *u, double *dudt, void *ws, size_t wsb, void *stream) {
+    return sp_rhs_wave_shell(s, u, dudt, 1, 1, ws, wsb, stream);
+}
+
+extern "C" sp_status sp_wave_interface(const sp_shell *a, double *da, const sp_shell *b, double *db, void *stream) {
+    if (!a || !b || !da || !db || a == b) return SP_ERR_INVALID_ARG;
+    if (!a->built || !b->built) return SP_ERR_NOT_BUILT;
+    if (a->Nt != b->Nt || a->Np != b->Np || fabs(a->rout - b->rin) > 1e-12 * fabs(a->rout)) return SP_ERR_INVALID_ARG;
+    const int n = a->Nt * a->Np;
+    g_sp_launches += 1;
+    k_wave_interface<<<(n + 127) / 128, 128, 0, (cudaStream_t)stream>>>(a->Nt, a->Np, a->Nr, b->Nr, a->d_sin_t, a->d_cos_t, a->d_sin_p,
+                                                                      a->d_cos_p, da, db);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
 
