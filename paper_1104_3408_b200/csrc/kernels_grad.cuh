@@ -414,6 +414,17 @@ __global__ void __launch_bounds__(KT == 3 ? 384 : 192, KT == 3 ? 1 : 2) k_grad_r
         }
     }
     __syncthreads();
+    if (NBUF == 1 && threadIdx.x < 2) {
+        // single-buffered (the plane pair of a large grid fills the SM's shared memory): the next item's planes cannot be staged
+        // under this item's products, but they can be pulled into L2 (one bulk prefetch per plane: a plane is Nr*Ntheta contiguous
+        // doubles), so that the exposed load phase of the next iteration reads L2 instead of HBM
+        const int nxt = it + gridDim.x;
+        if (nxt < p.nitems && !((nplane * 8) & 15)) {
+            const int mu_ = nxt / Nt, j_ = nxt - mu_ * Nt;
+            const double *up = p.u + mu_ * npts + (size_t)(j_ + (threadIdx.x ? Nt : 0)) * plane;
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(up), "r"(nplane * 8) : "memory");
+        }
+    }
     for (int task = warp; task < ntasks; task += nwarps) {
         const int it_ = task / kgroups, kg = task - it_ * kgroups;
         const int kt0 = kg * KT;
