@@ -152,6 +152,10 @@ sp_status sp_wave_interface(const sp_shell *inner, double *dudt_inner_dev, const
  * SP_ERR_INVALID_ARG. */
 sp_status sp_wave_dt(const sp_shell *shell, double lambda, double *dt_out);
 
+/* Graded scalar filter Yg, eq. (59): component mu of the 50-field GHG state keeps the degrees l <= L + d(u^mu),
+ * d = its number of spatial indices (g_tt: 0, g_tx: 1, g_xx: 2, ...; d_iab adds one), capped at the grid's Ntheta - 1.  Host only. */
+sp_status sp_ghg_graded_degree(const sp_shell *shell, int field, int *L_out);
+
 /* y <- a*x + b*y over n doubles (the RK4 combination steps of config 5). */
 sp_status sp_axpby(double a, const double *x_dev, double b, double *y_dev, size_t n, void *cuda_stream);
 

@@ -8,7 +8,7 @@ _lib = None
 # every symbol include/spshell.h declares
 EXPORTED_SYMBOLS = [
     "sp_shell_create", "sp_shell_destroy", "sp_build_matrices", "sp_workspace_bytes", "sp_cartesian_gradient",
-    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_rhs_wave_shell", "sp_wave_interface", "sp_wave_dt", "sp_axpby", "sp_rk4_stage", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
+    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_rhs_wave_shell", "sp_wave_interface", "sp_wave_dt", "sp_axpby", "sp_rk4_stage", "sp_ghg_graded_degree", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
     "sp_status_string", "sp_profile_enable", "sp_profile_read", "sp_launch_count",
 ]
 
@@ -50,6 +50,7 @@ def lib():
         L.sp_axpby.argtypes = [C.c_double, C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rk4_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_size_t,
                                    C.c_void_p]
+        L.sp_ghg_graded_degree.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int)]
         L.sp_ghg_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
         L.sp_rhs_ghg.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_ghg_init.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -245,6 +246,12 @@ class Shell:
         """dt = lambda * min(dx), eq. 63 (sp_wave_dt)."""
         v = C.c_double()
         _check(lib().sp_wave_dt(self._h, float(lam), C.byref(v)), "sp_wave_dt")
+        return v.value
+
+    def ghg_graded_degree(self, field):
+        """Kept degree of component `field` under the graded Yg filter, eq. 59 (sp_ghg_graded_degree)."""
+        v = C.c_int()
+        _check(lib().sp_ghg_graded_degree(self._h, int(field), C.byref(v)), "sp_ghg_graded_degree")
         return v.value
 
     def ghg_workspace_bytes(self):

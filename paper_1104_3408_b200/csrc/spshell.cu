@@ -1207,6 +1207,14 @@ extern "C" sp_status sp_wave_dt(const sp_shell *s, double lambda, double *dt) {
     return SP_OK;
 }
 
+extern "C" sp_status sp_ghg_graded_degree(const sp_shell *s, int field, int *L_out) {
+    if (!s || !L_out || field < 0 || field >= 50) return SP_ERR_INVALID_ARG;
+    static const int ab[10] = {0, 1, 1, 1, 2, 2, 2, 2, 2, 2};            // tt, tx, ty, tz, xx, xy, xz, yy, yz, zz
+    const int d = ab[field % 10] + (field >= 20 ? 1 : 0);                 // d_iab carries one more spatial index
+    *L_out = std::min(s->L + d, s->Nt - 1);
+    return SP_OK;
+}
+
 extern "C" sp_status sp_axpby(double a, const double *x, double b, double *y, size_t n, void *stream) {
     if (!x || !y) return SP_ERR_INVALID_ARG;
     if (n == 0) return SP_OK;

@@ -15,12 +15,6 @@ def ghg_tensors():
     ]
 
 
-def spatial_degree():
-    """d(u^mu) of PAPER.md:441: the number of spatial indices of each of the 50 Cartesian components."""
-    ab = [0, 1, 1, 1, 2, 2, 2, 2, 2, 2]
-    return ab + ab + [1 + q for _ in range(3) for q in ab]
-
-
 def scalar_tensors(fields):
     return [{"name": f"u{q}", "rank": 0, "dims": (), "sym": (-1, -1), "fields": [q]} for q in fields]
 
@@ -40,12 +34,11 @@ class GhgRK4:
         elif filter == "Y":
             self.passes = [(shell, scalar_tensors(range(50)))]
         elif filter == "Yg":
-            deg = spatial_degree()
+            kept = [shell.ghg_graded_degree(q) for q in range(50)]      # eq. 59, evaluated behind the ABI
             self.passes = []
-            for dgr in range(4):
-                L = min(shell.L + dgr, shell.Nt - 1)
-                shd = shell if dgr == 0 else Shell(shell.Nr, shell.Nt, shell.Np, shell.r_in, shell.r_out, L)
-                self.passes.append((shd, scalar_tensors([q for q in range(50) if deg[q] == dgr])))
+            for L in sorted(set(kept)):
+                shd = shell if L == shell.L else Shell(shell.Nr, shell.Nt, shell.Np, shell.r_in, shell.r_out, L)
+                self.passes.append((shd, scalar_tensors([q for q in range(50) if kept[q] == L])))
         else:
             raise ValueError("filter must be 'Yn', 'Y' or 'Yg'")
         self.passes = [(shd, t, shd.make_descs(t)) for shd, t in self.passes]

@@ -157,7 +157,7 @@ def test_graded_Yg_filter_parity():
     """Yg-filter (eq. 59): component mu is filtered as a scalar keeping l <= L + d(u^mu).  GPU: the same kernels with the
     tables of four shells; oracle: its scalar filter called per degree."""
     import torch
-    from paper_1104_3408_b200.ghg import GhgRK4, scalar_tensors, spatial_degree
+    from paper_1104_3408_b200.ghg import GhgRK4, scalar_tensors
     Nr, Nt, Np, L = 7, 9, 18, 4
     u = np.random.default_rng(9).standard_normal((50, Np, Nt, Nr))
     sh = _shell(Nr, Nt, Np, L=L)
@@ -166,7 +166,8 @@ def test_graded_Yg_filter_parity():
     rk = GhgRK4(sh, z4, z12, filter="Yg")
     v = torch.from_numpy(u).cuda()
     rk.filter(v)
-    deg = spatial_degree()
+    ab = [0, 1, 1, 1, 2, 2, 2, 2, 2, 2]                       # d(u^mu), written out here independently of the library
+    deg = ab + ab + [1 + q for _ in range(3) for q in ab]
     want = u.copy()
     for d in range(4):
         fields = [q for q in range(50) if deg[q] == d]

@@ -322,6 +322,8 @@ def test_shell_too_large_for_the_plane_kernels_is_refused_and_extreme_small_shel
     {"SP_THETA_NT": "3", "SP_GRAD_KT": "3", "SP_GRAD_NWARPS": "4", "SP_PHI_NC": "64", "SP_PHI_MSPLIT": "1"},
     {"SP_THETA_NT": "23", "SP_THETA_FOLD": "0"},
     {"SP_THETA_NT": "21", "SP_PHI_MSPLIT": "2"},
+    {"SP_FUSE": "2", "SP_FUSE_NBUF": "2", "SP_GRAD_CHUNK": "3"},
+    {"SP_FUSE": "1", "SP_FAN_NC4": "1", "SP_FAN_THREADS": "256", "SP_FSYN_NW": "8", "SP_THETA_TUNE": "1"},
 ])
 def test_tuning_overrides_keep_parity(env):
     """Every kernel variant the environment overrides can select (README, "tuning overrides") computes the same numbers: the

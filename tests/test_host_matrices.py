@@ -75,10 +75,18 @@ def test_filter_matrices_equatorial_reflection(Nt, L):
 
 
 def test_ghg_spatial_degree_and_layout():
-    """Host logic of the GHG driver: d(u^mu) of PAPER.md:441 (g_tt 0, g_tx 1, g_xx 2; d_iab one more) and the tensor layout."""
-    from paper_1104_3408_b200.ghg import ghg_tensors, spatial_degree
-    d = spatial_degree()
-    assert len(d) == 50 and d[0] == 0 and d[1] == 1 and d[4] == 2 and d[20] == 1 and d[21] == 2 and d[24] == 3
+    """Host logic of the GHG path: the graded kept degree L + d(u^mu) of eq. 59 (g_tt 0, g_tx 1, g_xx 2; d_iab one
+    more spatial index), evaluated behind the ABI (sp_ghg_graded_degree), capped at Ntheta - 1; and the tensor layout."""
+    from paper_1104_3408_b200 import Shell
+    from paper_1104_3408_b200.binding import SpError
+    from paper_1104_3408_b200.ghg import ghg_tensors
+    sh = Shell(7, 12, 24, 1.0, 2.0, 5, build=False)
+    d = [sh.ghg_graded_degree(q) - 5 for q in range(50)]
+    assert d[0] == 0 and d[1] == 1 and d[4] == 2 and d[20] == 1 and d[21] == 2 and d[24] == 3
     assert [d.count(q) for q in range(4)] == [2, 9, 21, 18]
+    assert [Shell(7, 12, 24, 1.0, 2.0, 10, build=False).ghg_graded_degree(q) for q in (0, 1, 4, 24)] == [10, 11, 11, 11]   # cap
+    import pytest
+    with pytest.raises(SpError):
+        sh.ghg_graded_degree(50)
     t = ghg_tensors()
     assert sorted(sum((x["fields"] for x in t), [])) == list(range(50))
