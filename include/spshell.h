@@ -50,7 +50,8 @@ typedef enum {
     SP_ERR_NOT_BUILT = 2,   /* a hot call before sp_build_matrices */
     SP_ERR_ALLOC = 3,       /* host or device allocation failed */
     SP_ERR_CUDA = 4,        /* a CUDA runtime call or kernel launch failed */
-    SP_ERR_UNSUPPORTED = 5  /* tensor index structure outside the supported set (see sp_tensor_desc) */
+    SP_ERR_UNSUPPORTED = 5, /* tensor index structure outside the supported set (see sp_tensor_desc) */
+    SP_ERR_SCRATCH_LIMIT = 6 /* sp_tensor_filter_noalloc: the call needs more than SP_NOALLOC_SCRATCH_BYTES of scratch */
 } sp_status;
 
 /* Per-tensor index layout: the paper's d(u^mu) made explicit.
@@ -104,6 +105,23 @@ sp_status sp_cartesian_gradient(const sp_shell *shell, const double *u_dev, int 
 sp_status sp_tensor_filter(const sp_shell *shell, const double *u_dev, double *out_dev, int nfields,
                            const sp_tensor_desc *tensors, int ntensors,
                            void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* The same filter for callers that cannot allocate or pass a workspace (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): sp_tensor_filter with its scratch (the spin-weight components and the two coefficient arrays)
+ * in a file-scope `static __device__` array of SP_NOALLOC_SCRATCH_BYTES = 32 MiB inside the library, which every GPU that loads
+ * the library holds until the process exits.  Arguments, layout, results and errors as sp_tensor_filter, minus the workspace.
+ *   - Allocates NOTHING on the device: no cudaMalloc / cudaFree / allocating library routine; the first call on a device resolves
+ *     the array's device address once (cudaGetSymbolAddress, with that device current) -- make that first call outside a capture.
+ *   - LIMIT: the call needs ncomp * (Nr Ntheta Nphi + 2 * roundup4(2L+1) * Nr Ntheta) * 8 bytes, ncomp = stored components of all
+ *     tensors (the `filter` figure of sp_workspace_bytes(shell, ncomp, ...)): e.g. the 50-field GHG state at 17 x 24 x 48
+ *     (20.9 MB) or the 5-field wave state at 33 x 64 x 128 (31.1 MB) fit, the GHG state at 33 x 48 x 96 (172 MB) does not.
+ *     Beyond the limit the call launches nothing and returns SP_ERR_SCRATCH_LIMIT; use sp_tensor_filter with your own workspace.
+ *   - SHARED: every call on a device uses the same array, which keeps the last call's contents.  Nothing in it has to start at
+ *     zero (every region is written before it is read within a call), so nothing is cleared; but two calls that OVERLAP on the GPU
+ *     (different streams, or concurrent host threads) race on it.  Calls on one stream, or ordered by events, are safe. */
+#define SP_NOALLOC_SCRATCH_BYTES (32u * 1024u * 1024u)
+sp_status sp_tensor_filter_noalloc(const sp_shell *shell, const double *u_dev, double *out_dev, int nfields,
+                                   const sp_tensor_desc *tensors, int ntensors, void *cuda_stream);
 
 /* First-order scalar wave RHS with characteristic boundaries (BASELINE.json config 5; W1-W3):
  * u = (psi, Pi, Phi_x, Phi_y, Phi_z);  d_t psi = -Pi, d_t Pi = -d_i Phi_i, d_t Phi_i = -d_i Pi; on the

@@ -8,7 +8,7 @@ _lib = None
 # every symbol include/spshell.h declares
 EXPORTED_SYMBOLS = [
     "sp_shell_create", "sp_shell_destroy", "sp_build_matrices", "sp_workspace_bytes", "sp_cartesian_gradient",
-    "sp_tensor_filter", "sp_rhs_first_order_wave", "sp_rhs_wave_shell", "sp_wave_interface", "sp_wave_dt", "sp_axpby", "sp_rk4_stage", "sp_ghg_graded_degree", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
+    "sp_tensor_filter", "sp_tensor_filter_noalloc", "sp_rhs_first_order_wave", "sp_rhs_wave_shell", "sp_wave_interface", "sp_wave_dt", "sp_axpby", "sp_rk4_stage", "sp_ghg_graded_degree", "sp_ghg_workspace_bytes", "sp_rhs_ghg", "sp_ghg_init", "sp_get_tuning", "sp_get_matrix", "sp_probe_fp64_peak",
     "sp_status_string", "sp_profile_enable", "sp_profile_read", "sp_launch_count",
 ]
 
@@ -43,6 +43,7 @@ def lib():
         L.sp_cartesian_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_tensor_filter.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(_TensorDesc), C.c_int,
                                        C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sp_tensor_filter_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(_TensorDesc), C.c_int, C.c_void_p]
         L.sp_rhs_first_order_wave.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_rhs_wave_shell.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sp_wave_interface.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -206,6 +207,19 @@ class Shell:
         ws = self._workspace(need, u.device) if workspace is None else _dev_f64(workspace, "workspace")
         _check(lib().sp_tensor_filter(self._h, u.data_ptr(), out.data_ptr(), nf, arr, nt, ws.data_ptr(), ws.numel() * 8,
                                       _stream_ptr(stream)), "sp_tensor_filter")
+        return out
+
+    NOALLOC_SCRATCH_BYTES = 32 * 1024 * 1024
+
+    def tensor_filter_noalloc(self, u, tensors, out, stream=None, descs=None):
+        """sp_tensor_filter_noalloc: the Yn filter with its scratch in the library's static 32 MiB device array -- no workspace
+        argument, no device allocation (the caller passes input and output).  Raises SpError (SP_ERR_SCRATCH_LIMIT) beyond the limit."""
+        u = _dev_f64(u, "u")
+        _dev_f64(out, "out")
+        nf = u.numel() // self.npts
+        arr, keep, nt = descs if descs is not None else self.make_descs(tensors)
+        _check(lib().sp_tensor_filter_noalloc(self._h, u.data_ptr(), out.data_ptr(), nf, arr, nt, _stream_ptr(stream)),
+               "sp_tensor_filter_noalloc")
         return out
 
     def rhs_first_order_wave(self, u, out=None, workspace=None, stream=None):

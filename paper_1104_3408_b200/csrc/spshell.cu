@@ -35,6 +35,7 @@ extern "C" const char *sp_status_string(sp_status s) {
         case SP_ERR_ALLOC: return "SP_ERR_ALLOC";
         case SP_ERR_CUDA: return "SP_ERR_CUDA";
         case SP_ERR_UNSUPPORTED: return "SP_ERR_UNSUPPORTED";
+        case SP_ERR_SCRATCH_LIMIT: return "SP_ERR_SCRATCH_LIMIT: the call needs more scratch than the 32 MiB static array of sp_tensor_filter_noalloc holds; use sp_tensor_filter with a workspace";
     }
     return "SP_ERR_?";
 }
@@ -1294,3 +1295,51 @@ extern "C" sp_status sp_profile_read(const sp_shell *s, double *ms7) {
 }
 
 extern "C" unsigned long long sp_launch_count(void) { return g_sp_launches; }
+
+// =================================================================================================
+// sp_tensor_filter_noalloc: the Yn filter with its scratch in a file-scope static device array (spshell.h).
+// In HOST code `g_sp_noalloc_scratch` is only a stand-in for the symbol, not a device address: the device address is resolved
+// once per device with cudaGetSymbolAddress (that device current) and that pointer is what the kernels get.
+// =================================================================================================
+static __device__ __align__(256) unsigned char g_sp_noalloc_scratch[SP_NOALLOC_SCRATCH_BYTES];
+
+#include <mutex>
+static const int SP_NOALLOC_MAXDEV = 64;
+static void *g_sp_noalloc_ptr[SP_NOALLOC_MAXDEV] = {};      // device address of the array on device d (null: not resolved yet)
+static std::mutex g_sp_noalloc_mu;
+
+static sp_status sp_noalloc_scratch(void **out) {
+    int dev = -1;
+    SP_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= SP_NOALLOC_MAXDEV) return SP_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_sp_noalloc_mu);
+    if (!g_sp_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_sp_noalloc_scratch) != cudaSuccess || !p) return SP_ERR_CUDA;
+        g_sp_noalloc_ptr[dev] = p;
+    }
+    *out = g_sp_noalloc_ptr[dev];
+    return SP_OK;
+}
+
+extern "C" sp_status sp_tensor_filter_noalloc(const sp_shell *s, const double *u, double *out, int nfields, const sp_tensor_desc *tens,
+                                              int ntens, void *stream) {
+    if (!s || !u || !out || nfields < 0 || ntens < 0 || (ntens > 0 && !tens)) return SP_ERR_INVALID_ARG;
+    if (!s->built) return SP_ERR_NOT_BUILT;
+    // scratch the call needs (as sp_tensor_filter computes it); malformed descriptors are left to sp_tensor_filter's own checks
+    size_t ndof = 0;
+    for (int t = 0; t < ntens; t++) {
+        if (tens[t].rank < 0 || tens[t].rank > 3 || !tens[t].field) return SP_ERR_INVALID_ARG;
+        const int tt = classify(tens[t]);
+        if (tt == -1) return SP_ERR_INVALID_ARG;
+        if (tt < 0) return SP_ERR_UNSUPPORTED;
+        ndof += (size_t)tt_ncomp(tt);
+    }
+    const size_t vec = (size_t)s->Nt * s->Nr;
+    const size_t need = ndof * (s->npts + 2 * (size_t)s->MC4 * vec) * sizeof(double);
+    if (need > (size_t)SP_NOALLOC_SCRATCH_BYTES) return SP_ERR_SCRATCH_LIMIT;      // nothing launched
+    void *ws = nullptr;
+    const sp_status e = sp_noalloc_scratch(&ws);
+    if (e != SP_OK) return e;
+    return sp_tensor_filter(s, u, out, nfields, tens, ntens, ws, (size_t)SP_NOALLOC_SCRATCH_BYTES, stream);
+}
