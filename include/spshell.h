@@ -30,7 +30,11 @@
  * shell may be issued on different streams (e.g. the gradient on one, the filter on another), but from ONE host thread
  * at a time: the shell's events are not protected against concurrent host threads.  Different shells are independent.
  *
- * ERRORS.  Every call returns an sp_status; nothing throws across the ABI.
+ * ERRORS.  Every call returns an sp_status; nothing throws across the ABI.  Argument errors are detected before anything is launched
+ * and leave the outputs untouched.  After any other non-OK status of a hot call (SP_ERR_CUDA: a launch failed mid-pipeline) the
+ * contents of the output arrays and of the workspace are UNDEFINED (earlier stages may have written intermediates into them, e.g. the
+ * gradient's d/dx slot); the shell's side stream is joined back into the caller's stream on every exit path, so a failed call
+ * cannot leave a CUDA graph capture forked.  Several shells may live in one process, built in any order, on the current device.
  */
 #ifndef SPSHELL_H
 #define SPSHELL_H

@@ -205,27 +205,26 @@ static inline size_t phi_smem_bytes(const PhiTiling &tl, int Mgrad = 0, int NC =
 }
 // column tile width: 64, or 32 when 64-wide tiles would give fewer than 2 CTAs per SM (small states: more, smaller CTAs keep
 // every SM busy and let several CTAs per SM overlap their load, product and store phases).  SP_PHI_NC overrides (experiments).
-extern int g_sp_num_sms;
-static inline int phi_ncol(int ncols, int nbatch) {
+static inline int phi_ncol(int ncols, int nbatch, int num_sms) {
     static const int forced = [] { const char *e = getenv("SP_PHI_NC"); return e ? atoi(e) : 0; }();
     if (forced == 32 || forced == 64) return forced;
     const long ctas64 = (long)((ncols + 63) / 64) * nbatch;
-    return ctas64 < 2L * g_sp_num_sms ? 32 : 64;
+    return ctas64 < 2L * num_sms ? 32 : 64;
 }
 
 // returns SP_ERR_UNSUPPORTED when the fast-path preconditions do not hold (caller falls back)
 static sp_status launch_phi_gemm(const double *A, int lda, int M, const PhiTiling &tl, int K, const double *B, long sBk, long sBb,
-                                 double *C, long sCm, long sCb, int ncols, int nbatch, cudaStream_t st,
+                                 double *C, long sCm, long sCb, int ncols, int nbatch, cudaStream_t st, int num_sms,
                                  const PhiGradEpi *ge = nullptr) {
     if ((sBk | sBb | sCm | sCb | (long)ncols) & 1) return SP_ERR_UNSUPPORTED;
     if (((uintptr_t)B | (uintptr_t)C) & 15) return SP_ERR_UNSUPPORTED;
     if (tl.mgroups > 4) return SP_ERR_UNSUPPORTED;
-    const int NC = phi_ncol(ncols, nbatch);
+    const int NC = phi_ncol(ncols, nbatch, num_sms);      // num_sms: SM count of the device the shell was built on
     // row blocks: products with two warp rows and many column tiles run as two CTAs of half the rows (measured: config 4
     // analysis -9 %, synthesis -4 %; config 3 d/dphi with the chain rule -7 %).  SP_PHI_MSPLIT overrides (experiments).
     static const int msplit_env = [] { const char *e = getenv("SP_PHI_MSPLIT"); return e ? atoi(e) : -1; }();
     const long ctas = (long)((ncols + NC - 1) / NC) * nbatch;
-    int zs = (tl.mgroups == 2 && ctas >= 8L * g_sp_num_sms) ? 2 : 1;
+    int zs = (tl.mgroups == 2 && ctas >= 8L * num_sms) ? 2 : 1;
     if (msplit_env >= 1) zs = (tl.mgroups % msplit_env == 0) ? msplit_env : 1;
     PhiTiling tz = tl;
     tz.mgroups = tl.mgroups / zs; tz.Mpad = tl.Mpad / zs;

@@ -22,7 +22,6 @@
         if (e_ != cudaSuccess) return SP_ERR_CUDA;   \
     } while (0)
 
-int g_sp_num_sms = 148;
 unsigned long long g_sp_launches = 0;
 
 static int round_up(int a, int b) { return (a + b - 1) / b * b; }
@@ -455,7 +454,6 @@ sp_status sp_configure_kernels(sp_shell *s) {
             }
         }
     }
-    g_sp_num_sms = s->num_sms;
     PhiTiling tmax = {6, 4, 4 * 6 * 8};
     const int pg = (int)phi_smem_bytes(tmax);
 #define SP_PGA(MTV)                                                                                             \
@@ -674,7 +672,7 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
             if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         } else {
             sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, du, plane, (long)s->npts, (int)plane, nf,
-                                          st, &ge);
+                                          st, s->num_sms, &ge);
             if (e != SP_OK) return e;
         }
         g_sp_launches += 2;
@@ -688,7 +686,7 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
     g_sp_launches += 2;
     double *dphi = (double *)ws;
     p.dphi = dphi;
-    sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
+    sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st, s->num_sms);
     if (e == SP_ERR_UNSUPPORTED)   // odd strides: generic global-memory kernel
         e = launch_gemm_cols<true>(s->d_g3, Np, Np, Np, u, plane, (long)s->npts, dphi, plane, (long)s->npts, (int)plane, nf, st);
     if (e != SP_OK) return e;
@@ -773,7 +771,7 @@ static void tt_components(int tt, int dof0, std::vector<ThetaComp> &out) {
 }
 
 template <bool INV>
-static void launch_pointwise(const std::vector<int> &types, const std::vector<TensorArgs> &targs, const std::vector<char> &sel,
+static sp_status launch_pointwise(const std::vector<int> &types, const std::vector<TensorArgs> &targs, const std::vector<char> &sel,
                              const sp_shell *s, const double *src, double *dst, cudaStream_t st) {
     const int T = 128;
     const unsigned nb = (unsigned)(((size_t)s->Nr * s->Nt * (s->Nt + 1) + T - 1) / T);
@@ -802,7 +800,8 @@ static void launch_pointwise(const std::vector<int> &types, const std::vector<Te
 #undef SP_PW
         g_sp_launches += 1;
     }
-    if (forked) sp_join(s, main_st);
+    if (forked && !sp_join(s, main_st)) return SP_ERR_CUDA;      // an unjoined side stream would also invalidate a graph capture
+    return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
 
 // ---- fused filter stages (kernels_fused.cuh) --------------------------------------------------------------------------------
@@ -1058,7 +1057,7 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     auto phi = [&](const sp_shell::PhiMat &pm, const double *B, long sBb, double *C, long sCb, int nb, cudaStream_t sx) -> sp_status {
         if (pm.M <= 0 || pm.K <= 0) return SP_OK;
         PhiTiling tl = {pm.MT, pm.mg, pm.Mpad};
-        sp_status e = launch_phi_gemm(pm.d, pm.K8, pm.M, tl, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, nb, sx);
+        sp_status e = launch_phi_gemm(pm.d, pm.K8, pm.M, tl, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, nb, sx, s->num_sms);
         if (e == SP_ERR_UNSUPPORTED)      // odd strides: generic global-memory kernel (same padded matrix)
             e = launch_gemm_cols<false>(pm.d, pm.K8, pm.M, pm.K, B, (long)vec, sBb, C, (long)vec, sCb, (int)vec, nb, sx);
         g_sp_launches += 1;
@@ -1067,7 +1066,7 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     sp_status e;
     // ---- F1: dyad projection (five-stage tensors)
     sp_mark(s, st, 3);
-    if (anyFanU) launch_pointwise<false>(types, targs, fanU, s, u, dofs, st);
+    if (anyFanU && (e = launch_pointwise<false>(types, targs, fanU, s, u, dofs, st)) != SP_OK) return e;
     sp_mark(s, st, 4);
     // ---- F1 + F2 fused; F2: phi analysis (eq. 33) on the folded rows: cosine block -> a_0..a_L, sine block -> b_1..b_L
     e = for_groups(types, targs, fanF, st, aux, [&](int tt, const TensorArgsGroup &tg, int n, cudaStream_t sx) { return fan_dispatch(tt, s, tg, n, u, coef1, sx, true); });
@@ -1125,7 +1124,7 @@ extern "C" sp_status sp_tensor_filter(const sp_shell *s, const double *u, double
     if (!aux.join()) return SP_ERR_CUDA;
     sp_mark(s, st, 7);
     // ---- F5: recombination (five-stage tensors)
-    if (anySynU) launch_pointwise<true>(types, targs, synU, s, dofs, out, st);
+    if (anySynU && (e = launch_pointwise<true>(types, targs, synU, s, dofs, out, st)) != SP_OK) return e;
     sp_mark(s, st, 8);
     return cudaGetLastError() == cudaSuccess ? SP_OK : SP_ERR_CUDA;
 }
