@@ -90,3 +90,32 @@ def test_ghg_spatial_degree_and_layout():
         sh.ghg_graded_degree(50)
     t = ghg_tensors()
     assert sorted(sum((x["fields"] for x in t), [])) == list(range(50))
+
+
+def test_header_compiles_as_plain_c_and_cxx(tmp_path):
+    """The boundary is a C ABI: include/spshell.h must compile as C99 and as C++ on its own, warnings as errors, and a C program
+    using every declared entry point must link against the library (no CUDA or C++ type may leak into the signatures)."""
+    import subprocess
+    hdr = os.path.join(ROOT, "include", "spshell.h")
+    src = tmp_path / "use.c"
+    src.write_text(
+        '#include "spshell.h"\n#include <stdio.h>\n'
+        "int main(void) {\n"
+        "    sp_shell *s = 0; double dt = 0; int L = 0; size_t g, f, w;\n"
+        "    if (sp_shell_create(9, 8, 16, 1.0, 3.0, 6, &s) != SP_OK) return 1;\n"
+        "    if (sp_wave_dt(s, 4.0, &dt) != SP_OK || !(dt > 0)) return 2;\n"
+        "    if (sp_ghg_graded_degree(s, 24, &L) != SP_OK || L != 7) return 3;\n"
+        "    if (sp_workspace_bytes(s, 1, &g, &f, &w) != SP_OK || f == 0) return 4;\n"
+        "    if (sp_tensor_filter_noalloc(s, 0, 0, 0, 0, 0, 0) != SP_ERR_INVALID_ARG) return 5;\n"
+        '    printf("%s %u\\n", sp_status_string(SP_ERR_SCRATCH_LIMIT), (unsigned)SP_NOALLOC_SCRATCH_BYTES);\n'
+        "    return sp_shell_destroy(s) == SP_OK ? 0 : 6;\n}\n")
+    inc = os.path.join(ROOT, "include")
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-fsyntax-only", "-x", "c", hdr], check=True)
+    subprocess.run(["g++", "-std=c++17", "-Wall", "-Wextra", "-Werror", "-fsyntax-only", "-x", "c++", hdr], check=True)
+    exe = tmp_path / "use"
+    libdir = os.path.dirname(binding.library_path())
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", inc, str(src), "-o", str(exe), "-L", libdir, "-lspshell",
+                    "-Wl,-rpath," + libdir], check=True)
+    r = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert r.returncode == 0, (r.returncode, r.stderr)
+    assert "SCRATCH_LIMIT" in r.stdout and str(32 * 1024 * 1024) in r.stdout
