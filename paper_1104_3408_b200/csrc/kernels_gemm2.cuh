@@ -14,6 +14,8 @@
 #include <cstdlib>
 #include <algorithm>
 
+// launches whose row blocks share an operand larger than this put the row-block index first in launch order
+#define SP_SPLIT_FAST_BYTES (32.0 * 1024 * 1024)
 #define PG_NCOL 64
 #define PG_KC 16
 #define PG_STAGES 3
@@ -45,11 +47,16 @@ struct PhiGradEpi {
 template <int MT, bool EPI_GRAD, int NC>
 __global__ void __launch_bounds__(NC * 8)
 k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const double *__restrict__ B, long sBk, long sBb,
-           double *__restrict__ C, long sCm, long sCb, int ncols, PhiGradEpi ge) {
+           double *__restrict__ C, long sCm, long sCb, int ncols, PhiGradEpi ge, int sfast) {
     extern __shared__ __align__(16) double sm[];
-    if (gridDim.z > 1) {                                // row blocks: this CTA owns rows [r0, r0 + Mpad / gridDim.z)
-        Mpad /= gridDim.z;
-        const int r0 = blockIdx.z * Mpad;
+    // grid = (column tiles, batch, row blocks), or with sfast (row blocks, column tiles, batch): the row blocks of one column tile
+    // read the same B columns; as neighbours in launch order (x fastest) the second one finds them in L2 instead of DRAM.  That pays
+    // when B is larger than L2 can keep; for small launches the simultaneous hits on the same lines cost more than they save.
+    const int nzs = sfast ? gridDim.x : gridDim.z, bz = sfast ? blockIdx.x : blockIdx.z;
+    const int bx = sfast ? blockIdx.y : blockIdx.x, by = sfast ? blockIdx.z : blockIdx.y;
+    if (nzs > 1) {                                // row blocks: this CTA owns rows [r0, r0 + Mpad / gridDim.x)
+        Mpad /= nzs;
+        const int r0 = bz * Mpad;
         M = min(M - r0, Mpad);
         A += (long)r0 * lda;
         C += (long)r0 * sCm;
@@ -62,9 +69,9 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
     double *As = sm, *Bs = sm + STG * stageA;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp / NG, ng = warp % NG;
-    const int c0 = blockIdx.x * NC;
-    const double *Bb = B + (long)blockIdx.y * sBb + c0;
-    double *Cb = C + (long)blockIdx.y * sCb + c0;
+    const int c0 = bx * NC;
+    const double *Bb = B + (long)by * sBb + c0;
+    double *Cb = C + (long)by * sCb + c0;
     const int nchunks = (K + KC - 1) / KC;
     const int colsleft = ncols - c0;                    // > 0, even
 
@@ -147,7 +154,7 @@ k_phi_gemm(const double *__restrict__ A, int lda, int M, int Mpad, int K, const 
         cp_async_wait<0>();
         __syncthreads();
         double *cs = sm;
-        double *Yb = ge.Y + (long)blockIdx.y * ge.sYb + c0;
+        double *Yb = ge.Y + (long)by * ge.sYb + c0;
 #pragma unroll
         for (int a = 0; a < MT; a++) {
             const int row = (mg * MT + a) * 8 + g;                       // longitude j
@@ -228,10 +235,13 @@ static sp_status launch_phi_gemm(const double *A, int lda, int M, const PhiTilin
     if (msplit_env >= 1) zs = (tl.mgroups % msplit_env == 0) ? msplit_env : 1;
     PhiTiling tz = tl;
     tz.mgroups = tl.mgroups / zs; tz.Mpad = tl.Mpad / zs;
-    dim3 grid((ncols + NC - 1) / NC, nbatch, zs), block(tz.mgroups * (NC / 16) * 32);
+    // row blocks fastest in launch order when the operand they share is too large to wait in L2 (see the kernel)
+    const int sfast = (zs > 1 && (double)K * ncols * nbatch * sizeof(double) > SP_SPLIT_FAST_BYTES) ? 1 : 0;
+    const dim3 grid = sfast ? dim3(zs, (ncols + NC - 1) / NC, nbatch) : dim3((ncols + NC - 1) / NC, nbatch, zs);
+    const dim3 block(tz.mgroups * (NC / 16) * 32);
 #define SP_PG(MTV, EPIV, SM, GE)                                                                                              \
-    if (NC == 32) k_phi_gemm<MTV, EPIV, 32><<<grid, block, SM, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, GE); \
-    else k_phi_gemm<MTV, EPIV, 64><<<grid, block, SM, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, GE);
+    if (NC == 32) k_phi_gemm<MTV, EPIV, 32><<<grid, block, SM, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, GE, sfast); \
+    else k_phi_gemm<MTV, EPIV, 64><<<grid, block, SM, st>>>(A, lda, M, tl.Mpad, K, B, sBk, sBb, C, sCm, sCb, ncols, GE, sfast);
     if (ge) {
         if ((ge->sYb & 1) || ((uintptr_t)ge->Y & 15)) return SP_ERR_UNSUPPORTED;
         const size_t sm = phi_smem_bytes(tz, std::min(M, tz.Mpad), NC);

@@ -21,14 +21,16 @@ template <int MT, int NC>
 __global__ void __launch_bounds__(NC * 8)
 k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, int lda, int J, int Mpad,
                 const double *__restrict__ U, long sUj, long sUb, double *__restrict__ X, double *__restrict__ Y, long sXb, int ncols,
-                PhiGradEpi ge) {
+                PhiGradEpi ge, int sfast) {
     extern __shared__ __align__(16) double sm[];
     constexpr int GF_PB = NC + 4, GF_PC = NC + 2, NG = NC / 16, HC = NC / 2;
     const int h = J >> 1, K = h + 1;
     int M = h + 1, r0 = 0;
-    if (gridDim.z > 1) {                                // row blocks: this CTA owns the rows j' in [r0, r0 + Mpad / gridDim.z) and their mirrors
-        Mpad /= gridDim.z;
-        r0 = blockIdx.z * Mpad;
+    const int nzs = sfast ? gridDim.x : gridDim.z, bz = sfast ? blockIdx.x : blockIdx.z;      // grid orders as in k_phi_gemm
+    const int bx = sfast ? blockIdx.y : blockIdx.x, by = sfast ? blockIdx.z : blockIdx.y;
+    if (nzs > 1) {                                // row blocks: this CTA owns the rows j' in [r0, r0 + Mpad / gridDim.x) and their mirrors
+        Mpad /= nzs;
+        r0 = bz * Mpad;
         M = min(M - r0, Mpad);
         Gm += (long)r0 * lda;
         Gp += (long)r0 * lda;
@@ -37,8 +39,8 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
     double *As = sm, *Bs = sm + GF_STAGES * stageA;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp / NG, ng = warp % NG;
-    const int c0 = blockIdx.x * NC;
-    const double *Ub = U + (long)blockIdx.y * sUb + c0;
+    const int c0 = bx * NC;
+    const double *Ub = U + (long)by * sUb + c0;
     const int colsleft = ncols - c0;
     const int nchunks = (K + GF_KC - 1) / GF_KC;
     const int mtiles = (M + 7) >> 3;
@@ -139,7 +141,7 @@ k_phi_grad_fold(const double *__restrict__ Gm, const double *__restrict__ Gp, in
         }
     }
     __syncthreads();
-    double *Xb = X + (long)blockIdx.y * sXb + c0, *Yb = Y + (long)blockIdx.y * sXb + c0;
+    double *Xb = X + (long)by * sXb + c0, *Yb = Y + (long)by * sXb + c0;
     const int npair = min(NC, colsleft) >> 1;                          // column pairs of this tile
     constexpr int UNR = 4;
     for (int q0 = tid; q0 < 2 * Mpad * HC; q0 += UNR * blockDim.x) {

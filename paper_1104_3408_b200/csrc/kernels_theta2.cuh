@@ -46,14 +46,15 @@ struct ThetaBatch2 { ThetaComp2 c[SP_THETA2_BATCH]; };
 template <int MT, int NT, bool CPLX>
 __global__ void __launch_bounds__(NT == 3 ? 384 : 896, 1)
 k_theta2(ThetaBatch2 comps, const double *__restrict__ F2, int L, int Nt, int Nt8, int Nr, int MC4, int mgroups, int rsplit,
-         const double *__restrict__ coef, double *__restrict__ cout) {
+         const double *__restrict__ coef, double *__restrict__ cout, int sfast) {
     extern __shared__ __align__(16) double sm[];
     constexpr int NMAT = CPLX ? 2 : 1, NARR = CPLX ? 4 : 2;
     const ThetaComp2 cmp = comps.c[blockIdx.y];
-    const int m = blockIdx.x;
-    // blockIdx.z = radial block * rsplit + row block: with rsplit = 2 a CTA owns half of the latitudes (rows of F^n_m), so its F tile
+    const int m = sfast ? blockIdx.x / rsplit : blockIdx.x;
+    // sfast (large launches): blockIdx.x = m * rsplit + row block (the row blocks of one (component, m, radial block) read the same coefficient rows: neighbours in
+    // launch order, so the second one finds them in L2), blockIdx.z = radial block; otherwise blockIdx.x = m, blockIdx.z = radial block * rsplit + row block: with rsplit = 2 a CTA owns half of the latitudes (rows of F^n_m), so its F tile
     // halves and two CTAs share an SM at large Ntheta; both row blocks read the same coefficient rows
-    const int zr = blockIdx.z % rsplit, k0 = (blockIdx.z / rsplit) * TH_RC;
+    const int zr = sfast ? blockIdx.x % rsplit : blockIdx.z % rsplit, k0 = (sfast ? blockIdx.z : blockIdx.z / rsplit) * TH_RC;
     const int Nt8c = Nt8 / rsplit, r0 = zr * Nt8c;                  // rows of this CTA
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int mg = warp % mgroups, ng = warp / mgroups, nwarps = blockDim.x >> 5;

@@ -348,10 +348,11 @@ static sp_status launch_theta2(const sp_shell *s, int v, const std::vector<Theta
             ThetaBatch2 b;
             const int nb = (int)std::min<size_t>(SP_THETA2_BATCH, lst.size() - c0);
             for (int q = 0; q < nb; q++) b.c[q] = lst[c0 + q];
-            const dim3 grid(s->L + 1, nb, gz * rsplit);
+            const int sfast = (rsplit > 1 && (double)nb * (pass ? 2 : 1) * s->MC * s->Nt * s->Nr * sizeof(double) > SP_SPLIT_FAST_BYTES) ? 1 : 0;
+            const dim3 grid = sfast ? dim3((s->L + 1) * rsplit, nb, gz) : dim3(s->L + 1, nb, gz * rsplit);
 #define SP_TH2(MTV, NTV)                                                                                                        \
-    if (pass) k_theta2<MTV, NTV, true><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, rsplit, coef1, coef2); \
-    else k_theta2<MTV, NTV, false><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, rsplit, coef1, coef2);
+    if (pass) k_theta2<MTV, NTV, true><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, rsplit, coef1, coef2, sfast); \
+    else k_theta2<MTV, NTV, false><<<grid, block, sm, st>>>(b, s->d_F, s->L, s->Nt, s->Nt8, s->Nr, s->MC4, mgroups, rsplit, coef1, coef2, sfast);
 #define SP_TH2M(NTV)                                                                                     \
     switch (MT) { case 1: SP_TH2(1, NTV) break; case 2: SP_TH2(2, NTV) break; case 3: SP_TH2(3, NTV) break; default: SP_TH2(4, NTV) break; }
             if (NT == 3) { SP_TH2M(3) } else { SP_TH2M(1) }
@@ -661,14 +662,15 @@ extern "C" sp_status sp_cartesian_gradient(const sp_shell *s, const double *u, i
             if (ctas < 4L * s->num_sms) zs = s->gf_mg;      // small states: one warp row per CTA (config 5: d/dphi 39 -> 29 us)
             if (zenv >= 1) zs = (s->gf_mg % zenv == 0) ? zenv : 1;
             const int mgc = s->gf_mg / zs;
-            const dim3 gridf(((int)plane + NC - 1) / NC, nf, zs);
+            const int sfast = (zs > 1 && (double)s->npts * nf * sizeof(double) > SP_SPLIT_FAST_BYTES) ? 1 : 0;
+            const dim3 gridf = sfast ? dim3(zs, ((int)plane + NC - 1) / NC, nf) : dim3(((int)plane + NC - 1) / NC, nf, zs);
             const size_t smf = gradfold_smem_bytes(s->gf_Mpad / zs, s->Np, NC);
             if (NC == 32)
                 k_phi_grad_fold<4, 32><<<gridf, mgc * 2 * 32, smf, st>>>(
-                    s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge);
+                    s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge, sfast);
             else
                 k_phi_grad_fold<4, 64><<<gridf, mgc * 4 * 32, smf, st>>>(
-                    s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge);
+                    s->d_gm, s->d_gp, s->gf_lda, Np, s->gf_Mpad, u, plane, (long)s->npts, du, ge.Y, (long)s->npts, (int)plane, ge, sfast);
             if (cudaGetLastError() != cudaSuccess) return SP_ERR_CUDA;
         } else {
             sp_status e = launch_phi_gemm(s->d_fd3p, s->Np8, Np, tl, Np, u, plane, (long)s->npts, du, plane, (long)s->npts, (int)plane, nf,
