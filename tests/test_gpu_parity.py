@@ -98,7 +98,7 @@ def test_filter_full(cid, white):
         assert _rel(got, u) < TOL
 
 
-@pytest.mark.parametrize("cid,radii,white", [(3, (0, 17), False), (3, (32,), True), (4, (0, 20, 40, 64), True), (5, (0, 16, 32), False),
+@pytest.mark.parametrize("cid,radii,white", [(3, (0, 17), False), (3, (32,), True), (4, (0, 20, 40, 64), True), (4, (7, 51), False), (5, (0, 16, 32), False),
                                              (5, (5,), True)])
 def test_filter_sampled_radii_full_size(cid, radii, white):
     """Full-size launch; the oracle filters whole spheres at sampled radii (F is independent of r).  The radii cover both
